@@ -1,0 +1,452 @@
+// C ABI of libsc_ivr (include/sc_ivr.h): argument validation, workspace carving, kernel sequencing.
+// No method arithmetic lives here except the host-side constants (reduced-coordinate scaling, the
+// normalisation of Eq. 11).
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+namespace {
+
+thread_local char g_create_err[512] = "";
+
+sc_ivr_status fail(sc_ivr_ctx *ctx, sc_ivr_status st, const char *fmt, ...) {
+  char *dst = ctx ? ctx->err : g_create_err;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) return fail(ctx, SC_IVR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline long long round_up_ll(long long x, long long a) { return (x + a - 1) / a * a; }
+
+long n_coeffs_expected(int F, int kind) {
+  if (kind == SC_IVR_PES_MORSE1D) return 4;
+  if (kind == SC_IVR_PES_QFF) return F + (long)F * (F + 1) * (F + 2) / 6 + (long)F * (F + 1) / 2;
+  if (kind == SC_IVR_PES_MORSE_UNCOUPLED) return 4L * F;
+  return -1;
+}
+
+// Workspace layout for one run.  Everything 256-byte aligned.
+struct Carve {
+  long long nbatch;     // trajectories per batch
+  long long nbp;        // nbatch rounded to the Fourier tile (z row stride)
+  int rows, zrows, kp;  // nsteps+1, rows padded to KC, k padded to TI
+  long long tiles_total;
+  size_t off_raw, off_z, off_W, off_partial, off_good, off_wg, off_E, off_ngood, total;
+};
+
+Carve carve(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
+  Carve c;
+  c.nbatch = nbatch;
+  c.nbp = round_up_ll(nbatch, SCI_TJ);
+  c.rows = ctx->nsteps + 1;
+  c.zrows = (int)round_up_ll(c.rows, SCI_KC);
+  c.kp = (int)round_up_ll(k, SCI_TI);
+  const long long nbatches = (ntraj + nbatch - 1) / nbatch;
+  c.tiles_total = nbatches * (c.nbp / SCI_TJ);
+  size_t o = 0;
+  c.off_raw = o; o = align_up(o + sizeof(double4) * (size_t)c.rows * (size_t)nbatch, 256);
+  c.off_z = o; o = align_up(o + sizeof(double2) * (size_t)c.zrows * (size_t)c.nbp, 256);
+  c.off_W = o; o = align_up(o + sizeof(double2) * (size_t)c.zrows * (size_t)c.kp, 256);
+  c.off_partial = o; o = align_up(o + sizeof(double) * (size_t)c.tiles_total * (size_t)c.kp, 256);
+  c.off_good = o; o = align_up(o + (size_t)ntraj, 256);
+  c.off_wg = o; o = align_up(o + sizeof(double) * (size_t)ntraj, 256);
+  c.off_E = o; o = align_up(o + sizeof(double) * (size_t)k, 256);
+  c.off_ngood = o; o = align_up(o + 64, 256);
+  c.total = o;
+  return c;
+}
+
+long long default_batch(const sc_ivr_ctx *ctx, long long ntraj, long long max_batch) {
+  if (max_batch <= 0) max_batch = 131072;
+  long long nb = ntraj < max_batch ? ntraj : max_batch;
+  if (nb < ntraj) {  // several batches: make each a whole number of kernel-A waves
+    nb = nb / ctx->wave * ctx->wave;
+    if (nb < ctx->wave) nb = ctx->wave;
+  }
+  return nb;
+}
+
+void fill_prop_params(const sc_ivr_ctx *ctx, PropParams &P, const double *chi) {
+  memset(&P, 0, sizeof(P));
+  const int F = ctx->F;
+  P.nstages = ctx->nstages;
+  for (int s = 0; s < ctx->nstages; s++) {
+    P.kick[s] = ctx->sb[s] * ctx->dt;
+    P.drift[s] = ctx->sa[s] * ctx->dt;
+  }
+  for (int a = 0; a < F; a++) {
+    const double sg = sqrt(ctx->gamma[a]);
+    P.sg[a] = sg;
+    P.isg[a] = 1.0 / sg;
+    P.mu[a] = ctx->gamma[a] / ctx->mass[a];
+    P.Peq[a] = chi ? chi[a] / sg : 0.0;
+    P.Qeq[a] = chi ? chi[F + a] * sg : 0.0;
+  }
+  P.coef = ctx->d_coef;
+  P.det_tol = ctx->det_tol;
+  P.det_stride = ctx->det_stride;
+}
+
+struct StageTimer {
+  sc_ivr_ctx *ctx;
+  cudaStream_t st;
+  bool on;
+  StageTimer(sc_ivr_ctx *c, cudaStream_t s) : ctx(c), st(s), on(c->timing != 0) {}
+  void begin() {
+    if (on) cudaEventRecord(ctx->ev[0], st);
+  }
+  void end(int slot) {  // synchronising: only used when timing is switched on
+    if (!on) return;
+    cudaEventRecord(ctx->ev[1], st);
+    cudaEventSynchronize(ctx->ev[1]);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]);
+    ctx->tms[slot] += ms;
+  }
+};
+
+}  // namespace
+
+extern "C" {
+
+const char *sc_ivr_last_error(const sc_ivr_ctx *ctx) { return ctx ? ctx->err : g_create_err; }
+
+sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const double *pes_coeffs, size_t n_coeffs,
+                            const double *gamma, double dt, int nsteps, const sc_ivr_options *opt) {
+  sc_ivr_ctx *ctx = nullptr;  // errors before allocation go to the thread-local message
+  if (!out) return fail(ctx, SC_IVR_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!pes_coeffs || !gamma) return fail(ctx, SC_IVR_EINVAL, "pes_coeffs/gamma is NULL");
+  if (F < 1) return fail(ctx, SC_IVR_EINVAL, "F = %d < 1", F);
+  if (F > SC_IVR_MAX_F) return fail(ctx, SC_IVR_EUNSUPPORTED, "F = %d > SC_IVR_MAX_F = %d", F, SC_IVR_MAX_F);
+  if (kind != SC_IVR_PES_MORSE1D && kind != SC_IVR_PES_QFF && kind != SC_IVR_PES_MORSE_UNCOUPLED)
+    return fail(ctx, SC_IVR_EUNSUPPORTED, "unknown PES kind %d", (int)kind);
+  if (kind == SC_IVR_PES_MORSE1D && F != 1) return fail(ctx, SC_IVR_EINVAL, "MORSE1D needs F = 1");
+  if ((long)n_coeffs != n_coeffs_expected(F, kind))
+    return fail(ctx, SC_IVR_EINVAL, "n_coeffs = %zu, expected %ld", n_coeffs, n_coeffs_expected(F, kind));
+  if (!(dt > 0.0) || !isfinite(dt)) return fail(ctx, SC_IVR_EINVAL, "dt must be > 0");
+  if (nsteps < 1) return fail(ctx, SC_IVR_EINVAL, "nsteps must be >= 1");
+  for (size_t i = 0; i < n_coeffs; i++)
+    if (!isfinite(pes_coeffs[i])) return fail(ctx, SC_IVR_EINVAL, "pes_coeffs[%zu] is not finite", i);
+  for (int a = 0; a < F; a++)
+    if (!(gamma[a] > 0.0) || !isfinite(gamma[a])) return fail(ctx, SC_IVR_EINVAL, "gamma[%d] must be > 0", a);
+  int integrator = opt ? opt->integrator : 0;
+  int det_stride = opt ? opt->det_stride : 1;
+  double det_tol = opt ? opt->det_tol : 1e-6;
+  if (det_stride == 0) det_stride = 1;
+  if (det_tol == 0.0) det_tol = 1e-6;
+  if (det_stride < 1 || !(det_tol > 0.0)) return fail(ctx, SC_IVR_EINVAL, "bad det_stride/det_tol");
+  if (integrator != 0 && integrator != 1) return fail(ctx, SC_IVR_EUNSUPPORTED, "unknown integrator %d", integrator);
+
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev < 1)
+    return fail(ctx, SC_IVR_ECUDA, "no CUDA device (%s): this library has no CPU fallback",
+                ce == cudaSuccess ? "device count 0" : cudaGetErrorString(ce));
+
+  ctx = new (std::nothrow) sc_ivr_ctx;
+  if (!ctx) return fail(nullptr, SC_IVR_ENOMEM, "out of host memory");
+  memset(ctx, 0, sizeof(*ctx));
+  ctx->F = F;
+  ctx->kind = (int)kind;
+  ctx->nsteps = nsteps;
+  ctx->dt = dt;
+  ctx->det_stride = det_stride;
+  ctx->det_tol = det_tol;
+  ctx->integrator = integrator;
+  for (int a = 0; a < F; a++) {
+    ctx->gamma[a] = gamma[a];
+    ctx->mass[a] = (kind == SC_IVR_PES_QFF) ? 1.0 : pes_coeffs[4 * a + 3];
+    if (!(ctx->mass[a] > 0.0)) {
+      delete ctx;
+      return fail(nullptr, SC_IVR_EINVAL, "mass[%d] must be > 0", a);
+    }
+  }
+  if (integrator == 0) {  // velocity-Verlet as "kick b then drift a" stages (R10)
+    ctx->nstages = 2;
+    ctx->sb[0] = 0.5; ctx->sa[0] = 1.0;
+    ctx->sb[1] = 0.5; ctx->sa[1] = 0.0;
+  } else {  // 4-stage 4th-order symplectic composition (table of McLachlan & Atela)
+    ctx->nstages = 4;
+    const double b[4] = {0.1344961992774310892, -0.2248198030794208058, 0.7563200005156682911, 0.3340036032863214255};
+    const double a[4] = {0.5153528374311229364, -0.085782019412973646, 0.4415830236164665242, 0.1288461583653841854};
+    for (int s = 0; s < 4; s++) { ctx->sb[s] = b[s]; ctx->sa[s] = a[s]; }
+  }
+  sc_ivr_status rc = SC_IVR_OK;
+  do {
+    if (cudaGetDevice(&ctx->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device) != cudaSuccess) {
+      rc = fail(nullptr, SC_IVR_ECUDA, "cannot query the CUDA device");
+      break;
+    }
+    const size_t nc = sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr);
+    std::vector<double> packed(nc + F);  // sqrt(gamma) rides behind the coefficients (for sc_ivr_eval_pes)
+    sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, packed.data());
+    for (int a = 0; a < F; a++) packed[nc + a] = sqrt(gamma[a]);
+    ctx->n_coef = nc;
+    if ((ce = cudaMalloc(&ctx->d_coef, sizeof(double) * (nc + F))) != cudaSuccess ||
+        (ce = cudaMemcpy(ctx->d_coef, packed.data(), sizeof(double) * (nc + F), cudaMemcpyHostToDevice)) != cudaSuccess) {
+      rc = fail(nullptr, SC_IVR_ECUDA, "coefficient upload: %s", cudaGetErrorString(ce));
+      break;
+    }
+    if (cudaEventCreate(&ctx->ev[0]) != cudaSuccess || cudaEventCreate(&ctx->ev[1]) != cudaSuccess) {
+      rc = fail(nullptr, SC_IVR_ECUDA, "event creation failed");
+      break;
+    }
+    ctx->wave = (long long)ctx->sm_count * sci_prop_blocks_per_sm(F, (int)kind) * sci_prop_traj_per_block(F);
+  } while (0);
+  if (rc != SC_IVR_OK) {
+    sc_ivr_destroy(ctx);
+    return rc;
+  }
+  *out = ctx;
+  return SC_IVR_OK;
+}
+
+void sc_ivr_destroy(sc_ivr_ctx *ctx) {
+  if (!ctx) return;
+  if (ctx->d_coef) cudaFree(ctx->d_coef);
+  if (ctx->ev[0]) cudaEventDestroy(ctx->ev[0]);
+  if (ctx->ev[1]) cudaEventDestroy(ctx->ev[1]);
+  delete ctx;
+}
+
+long long sc_ivr_min_batch(const sc_ivr_ctx *ctx) { return ctx ? ctx->wave : 0; }
+
+size_t sc_ivr_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, long long max_batch) {
+  if (!ctx || ntraj < 1 || k < 1) return 0;
+  return carve(ctx, ntraj, k, default_batch(ctx, ntraj, max_batch)).total;
+}
+
+size_t sc_ivr_host_staging_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k) {
+  if (!ctx || ntraj < 1 || k < 1) return 0;
+  return align_up(sizeof(double) * 2 * (size_t)ctx->F * (size_t)ntraj, 256) + align_up(sizeof(double) * (size_t)ntraj, 256) +
+         align_up(sizeof(double) * (size_t)k, 256);
+}
+
+void sc_ivr_set_timing(sc_ivr_ctx *ctx, int on) {
+  if (ctx) ctx->timing = on;
+}
+
+sc_ivr_status sc_ivr_last_timings(sc_ivr_ctx *ctx, double out[6]) {
+  if (!ctx || !out) return SC_IVR_EINVAL;
+  for (int i = 0; i < 6; i++) out[i] = ctx->tms[i];
+  return SC_IVR_OK;
+}
+
+sc_ivr_status sc_ivr_fp64_probe(int mode, int iters, double *flops_out, double *ms_out) {
+  sc_ivr_ctx *ctx = nullptr;
+  if (!flops_out || !ms_out || iters < 1 || (mode != 0 && mode != 1)) return fail(ctx, SC_IVR_EINVAL, "bad probe arguments");
+  CU(sci_fp64_probe(mode, iters, flops_out, ms_out));
+  return SC_IVR_OK;
+}
+
+sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chi,
+                         const double *E, int k, double *I_out, long long *n_good_out, void *workspace,
+                         size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!p0q0 || !chi || !E || !I_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (ntraj < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "ntraj and k must be >= 1");
+  if (((uintptr_t)workspace & 255) != 0) return fail(ctx, SC_IVR_EINVAL, "workspace must be 256-byte aligned");
+  for (int a = 0; a < 2 * ctx->F; a++)
+    if (!isfinite(chi[a])) return fail(ctx, SC_IVR_EINVAL, "chi[%d] is not finite", a);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int F = ctx->F;
+
+  // largest batch (whole kernel-A waves) whose workspace fits
+  long long nbatch = default_batch(ctx, ntraj, 0);
+  Carve cv = carve(ctx, ntraj, k, nbatch);
+  while (cv.total > workspace_bytes && nbatch > ctx->wave) {
+    long long nx = nbatch / 2 / ctx->wave * ctx->wave;
+    if (nx < ctx->wave) nx = ctx->wave;
+    nbatch = nx;
+    cv = carve(ctx, ntraj, k, nbatch);
+  }
+  if (cv.total > workspace_bytes)
+    return fail(ctx, SC_IVR_EINVAL, "workspace too small: %zu bytes given, %zu needed for the minimum batch of %lld", workspace_bytes,
+                cv.total, nbatch);
+
+  char *ws = (char *)workspace;
+  double4 *raw = (double4 *)(ws + cv.off_raw);
+  double2 *z = (double2 *)(ws + cv.off_z);
+  double2 *W = (double2 *)(ws + cv.off_W);
+  double *partial = (double *)(ws + cv.off_partial);
+  unsigned char *good = (unsigned char *)(ws + cv.off_good);
+  double *wg = (double *)(ws + cv.off_wg);
+  double *E_dev = (double *)(ws + cv.off_E);
+  long long *ngood = (long long *)(ws + cv.off_ngood);
+
+  for (int i = 0; i < 6; i++) ctx->tms[i] = 0.0;
+  StageTimer tm(ctx, st);
+  double launches = 0;
+
+  CU(cudaMemcpyAsync(E_dev, E, sizeof(double) * k, cudaMemcpyHostToDevice, st));
+  tm.begin();
+  CU(sci_launch_twiddle(E_dev, k, cv.kp, cv.zrows, ctx->dt, W, st));
+  tm.end(2);
+  launches += 1;
+
+  PropParams P;
+  fill_prop_params(ctx, P, chi);
+  P.p0q0 = p0q0;
+  P.stride = ntraj;
+  P.nsteps = ctx->nsteps;
+  P.raw = raw;
+  P.raw_stride = cv.nbatch;
+
+  long long tile0 = 0;
+  for (long long j0 = 0; j0 < ntraj; j0 += nbatch) {
+    const long long nb = (ntraj - j0 < nbatch) ? ntraj - j0 : nbatch;
+    const long long zcols = round_up_ll(nb, SCI_TJ);
+    P.j0 = j0;
+    P.nb = nb;
+    P.good = good + j0;
+    tm.begin();
+    CU(sci_launch_propagate(F, ctx->kind, P, st));
+    tm.end(0);
+    tm.begin();
+    CU(sci_launch_zassemble(raw, cv.nbatch, nb, ctx->nsteps, z, cv.nbp, zcols, cv.zrows, nullptr, st));
+    tm.end(1);
+    tm.begin();
+    CU(sci_launch_weights(weights ? weights + j0 : nullptr, good + j0, nb, wg + j0, st));
+    tm.end(4);
+    tm.begin();
+    CU(sci_launch_fourier(z, cv.nbp, zcols, cv.zrows, W, cv.kp, nb, wg + j0, partial + tile0 * cv.kp, nullptr, k, st));
+    tm.end(3);
+    tile0 += zcols / SCI_TJ;
+    launches += 4;
+  }
+  tm.begin();
+  CU(sci_launch_count_good(good, ntraj, ngood, 0, st));
+  const double T = (double)ctx->nsteps * ctx->dt;
+  const double norm = ctx->dt * ctx->dt / (pow(2.0 * M_PI, F + 1) * T);  // Eq. 11 with R4's dt^2; 1/n_good on the device
+  CU(sci_launch_final(partial, tile0, cv.kp, k, ngood, norm, I_out, st));
+  tm.end(4);
+  launches += 2;
+  ctx->tms[5] = launches;
+
+  if (n_good_out) {
+    long long ng = 0;
+    CU(cudaMemcpyAsync(&ng, ngood, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    *n_good_out = ng;
+    if (ng == 0) return fail(ctx, SC_IVR_ENOGOOD, "every trajectory was rejected");
+  }
+  return SC_IVR_OK;
+}
+
+sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chi,
+                              const double *E, int k, double *I_out, long long *n_good_out, void *workspace,
+                              size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!p0q0 || !I_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (ntraj < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "ntraj and k must be >= 1");
+  const size_t stg = sc_ivr_host_staging_bytes(ctx, ntraj, k);
+  if (workspace_bytes < stg) return fail(ctx, SC_IVR_EINVAL, "workspace smaller than the host staging area");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  char *ws = (char *)workspace;
+  const size_t n_pq = sizeof(double) * 2 * (size_t)ctx->F * (size_t)ntraj;
+  double *d_pq = (double *)ws;
+  double *d_w = (double *)(ws + align_up(n_pq, 256));
+  double *d_I = (double *)((char *)d_w + align_up(sizeof(double) * (size_t)ntraj, 256));
+  CU(cudaMemcpyAsync(d_pq, p0q0, n_pq, cudaMemcpyHostToDevice, st));
+  if (weights) CU(cudaMemcpyAsync(d_w, weights, sizeof(double) * (size_t)ntraj, cudaMemcpyHostToDevice, st));
+  long long ng = 0;
+  sc_ivr_status rc = sc_ivr_run(ctx, d_pq, weights ? d_w : nullptr, ntraj, chi, E, k, d_I, &ng, ws + stg, workspace_bytes - stg, st);
+  if (n_good_out) *n_good_out = ng;
+  if (rc != SC_IVR_OK && rc != SC_IVR_ENOGOOD) return rc;
+  CU(cudaMemcpyAsync(I_out, d_I, sizeof(double) * (size_t)k, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  return rc;
+}
+
+size_t sc_ivr_propagate_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int nsteps_run) {
+  if (!ctx || ntraj < 1 || nsteps_run < 0) return 0;
+  return align_up(sizeof(double4) * (size_t)(nsteps_run + 1) * (size_t)ntraj, 256);
+}
+
+sc_ivr_status sc_ivr_propagate(sc_ivr_ctx *ctx, const double *p0q0, long long ntraj, int nsteps_run, const double *chi,
+                               double *pq_out, double *S_out, double *M_out, double *theta_out, unsigned char *good_out,
+                               double *z_out, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!p0q0) return fail(ctx, SC_IVR_EINVAL, "p0q0 is NULL");
+  if (ntraj < 1 || nsteps_run < 0) return fail(ctx, SC_IVR_EINVAL, "ntraj must be >= 1 and nsteps_run >= 0");
+  const bool need_raw = theta_out || z_out;
+  if (need_raw && (!workspace || workspace_bytes < sc_ivr_propagate_workspace_bytes(ctx, ntraj, nsteps_run)))
+    return fail(ctx, SC_IVR_EINVAL, "workspace too small for theta_out/z_out");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  PropParams P;
+  fill_prop_params(ctx, P, chi);
+  P.p0q0 = p0q0;
+  P.stride = ntraj;
+  P.j0 = 0;
+  P.nb = ntraj;
+  P.nsteps = nsteps_run;
+  P.raw = need_raw ? (double4 *)workspace : nullptr;
+  P.raw_stride = ntraj;
+  P.good = good_out;
+  P.pq_out = pq_out;
+  P.S_out = S_out;
+  P.M_out = M_out;
+  CU(sci_launch_propagate(ctx->F, ctx->kind, P, st));
+  if (need_raw)
+    CU(sci_launch_zassemble((const double4 *)workspace, ntraj, ntraj, nsteps_run, (double2 *)z_out, ntraj, ntraj, nsteps_run + 1,
+                            theta_out, st));
+  return SC_IVR_OK;
+}
+
+sc_ivr_status sc_ivr_eval_pes(sc_ivr_ctx *ctx, const double *q, long long n, double *V_out, double *g_out, double *H_out,
+                              void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!q || !V_out || !g_out || !H_out) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (n < 1) return fail(ctx, SC_IVR_EINVAL, "n must be >= 1");
+  CU(sci_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
+                         (cudaStream_t)cuda_stream));
+  return SC_IVR_OK;
+}
+
+size_t sc_ivr_fourier_workspace_bytes(const sc_ivr_ctx *ctx, long long n, int k) {
+  if (!ctx || n < 1 || k < 1) return 0;
+  const size_t zrows = (size_t)round_up_ll(ctx->nsteps + 1, SCI_KC), ncp = (size_t)round_up_ll(n, SCI_TJ);
+  const size_t kp = (size_t)round_up_ll(k, SCI_TI);
+  return align_up(sizeof(double2) * zrows * ncp, 256) + align_up(sizeof(double2) * zrows * kp, 256) + align_up(sizeof(double) * k, 256);
+}
+
+sc_ivr_status sc_ivr_fourier(sc_ivr_ctx *ctx, const double *zin, long long n, const double *E, int k, double *A_out,
+                             void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!zin || !E || !A_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (n < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "n and k must be >= 1");
+  if (workspace_bytes < sc_ivr_fourier_workspace_bytes(ctx, n, k)) return fail(ctx, SC_IVR_EINVAL, "workspace too small");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int rows = ctx->nsteps + 1;
+  const int zrows = (int)round_up_ll(rows, SCI_KC), kp = (int)round_up_ll(k, SCI_TI);
+  const long long ncp = round_up_ll(n, SCI_TJ);
+  char *ws = (char *)workspace;
+  double2 *z = (double2 *)ws;
+  double2 *W = (double2 *)(ws + align_up(sizeof(double2) * (size_t)zrows * (size_t)ncp, 256));
+  double *E_dev = (double *)((char *)W + align_up(sizeof(double2) * (size_t)zrows * (size_t)kp, 256));
+  CU(cudaMemsetAsync(z, 0, sizeof(double2) * (size_t)zrows * (size_t)ncp, st));
+  CU(cudaMemcpy2DAsync(z, sizeof(double2) * ncp, zin, sizeof(double2) * n, sizeof(double2) * n, rows, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpyAsync(E_dev, E, sizeof(double) * k, cudaMemcpyHostToDevice, st));
+  CU(sci_launch_twiddle(E_dev, k, kp, zrows, ctx->dt, W, st));
+  CU(sci_launch_fourier(z, ncp, ncp, zrows, W, kp, n, nullptr, nullptr, (double2 *)A_out, k, st));
+  return SC_IVR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,78 @@
+// Internal declarations shared by the translation units of libsc_ivr (CUDA path only; the CPU
+// oracle under oracle/ shares nothing with this directory).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sc_ivr.h"
+
+#define SCI_MAXF SC_IVR_MAX_F
+#define SCI_MAX_STAGES 4
+
+// ---- kernel A (propagate) parameters: passed by value, read through the constant bank ----------
+// All per-mode quantities are in REDUCED coordinates Q_k = sqrt(gamma_k) q_k, P_k = p_k / sqrt(gamma_k)
+// (pin P8): the Herman-Kluk matrix becomes
+// 2K = (M_qq + M_pp) + i (M_pq - M_qp) with no gamma factors.
+struct PropParams {
+  const double *p0q0;   // [2F][stride]
+  long long stride;     // ntraj of the caller's array
+  long long j0;         // first trajectory of this launch
+  long long nb;         // trajectories in this launch
+  int nsteps;
+  int det_stride;
+  double det_tol;
+  int nstages;
+  double kick[SCI_MAX_STAGES];   // b_i * dt
+  double drift[SCI_MAX_STAGES];  // a_i * dt
+  double sg[SCI_MAXF];           // sqrt(gamma)
+  double isg[SCI_MAXF];          // 1/sqrt(gamma)
+  double mu[SCI_MAXF];           // gamma/mass: dQ/dt = mu P, T = 1/2 sum mu P^2
+  double Peq[SCI_MAXF], Qeq[SCI_MAXF];
+  const double *coef;            // packed reduced PES coefficients (device)
+  double4 *raw;                  // [nsteps+1][raw_stride]: (ln|<chi|pq>|, S + arg<chi|pq>, Re det 2K, Im det 2K); may be NULL
+  long long raw_stride;
+  unsigned char *good;           // [nb]; may be NULL
+  // debug outputs (may be NULL), indexed by the GLOBAL trajectory number j0 + jj with stride `stride`
+  double *pq_out, *S_out, *M_out;
+};
+
+struct sc_ivr_ctx {
+  int F, kind, nsteps, det_stride, integrator;
+  double dt, det_tol;
+  double gamma[SCI_MAXF], mass[SCI_MAXF];
+  int nstages;
+  double sa[SCI_MAX_STAGES], sb[SCI_MAX_STAGES];
+  double *d_coef;
+  size_t n_coef;
+  int device, sm_count;
+  long long wave;  // trajectories one full wave of kernel A holds (batch granularity)
+  char err[512];
+  int timing;
+  double tms[6];
+  // timing events
+  cudaEvent_t ev[2];
+};
+
+// kernel A launchers (propagate.cu)
+int sci_prop_traj_per_block(int F);
+int sci_prop_blocks_per_sm(int F, int kind);
+size_t sci_pack_coeffs(int F, int kind, const double *coeffs, const double *gamma, double *out /*may be NULL: size query*/);
+cudaError_t sci_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st);
+cudaError_t sci_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q,
+                                long long n, double *V, double *g, double *H, cudaStream_t st);
+
+// spectrum stage (spectrum.cu)
+#define SCI_TJ 128  // trajectories per Fourier tile
+#define SCI_TI 64   // energies per Fourier tile
+#define SCI_KC 16   // time samples per pipeline stage
+cudaError_t sci_launch_zassemble(const double4 *raw, long long raw_stride, long long nb, int nsteps, double2 *z,
+                                 long long zstride, long long zcols, int zrows, double *theta_out, cudaStream_t st);
+cudaError_t sci_launch_twiddle(const double *E_dev, int k, int kp, int rows, double dt, double2 *W, cudaStream_t st);
+cudaError_t sci_launch_fourier(const double2 *z, long long zstride, long long zcols, int zrows, const double2 *W, int kp, long long nb,
+                               const double *wg /*[nb] weight*good*/, double *partial /*[tiles][kp]*/,
+                               double2 *A_out /*debug [nb][k] or NULL*/, int k, cudaStream_t st);
+cudaError_t sci_launch_weights(const double *w, const unsigned char *good, long long n, double *wg, cudaStream_t st);
+cudaError_t sci_launch_count_good(const unsigned char *good, long long n, long long *ngood, int accumulate, cudaStream_t st);
+cudaError_t sci_launch_final(const double *partial, long long ntiles, int kp, int k, const long long *ngood, double norm_no_ngood,
+                             double *I_out, cudaStream_t st);
+cudaError_t sci_fp64_probe(int mode, int iters, double *flops, double *ms);

@@ -1,0 +1,590 @@
+// Kernel A: fused PES (a1) + symplectic step (a2) + monodromy (a3) + action (a4) + Herman-Kluk
+// determinant (a5) + coherent-state overlap exponent (a6) + det M quality flag (a7).
+//
+// Mapping: F lanes per trajectory, G = floor(32/F) trajectories per warp.
+// Lane a of a group owns (P_a, Q_a), its share S_a of the action and the two tangent vectors
+// d(P,Q)/dP0_a and d(P,Q)/dQ0_a (columns a and F+a of the monodromy matrix, 2F doubles each), all in
+// registers.  The tangent map of a kick needs the full Hessian, so the lanes of a group compute
+// disjoint Hessian entries and exchange them through a per-group shared-memory slot.
+// Column a of the Herman-Kluk matrix lives entirely on lane a, so det K is a column-distributed
+// elimination with column pivoting: the pivot column is broadcast with __shfl_sync from a dynamic
+// source lane, no data is ever swapped.
+//
+// Everything runs in reduced coordinates Q = sqrt(gamma) q, P = p / sqrt(gamma).
+#include "common.cuh"
+
+namespace {
+
+constexpr int kThreads = 128;
+
+__device__ __forceinline__ double fast_rcp(double x) {
+  // MUFU.RCP64H seed (2^-23 relative) + two Newton steps: ~1 ulp for normal x, no slow path.
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  return r;
+}
+
+template <int F>
+struct Geo {
+  static constexpr int G = 32 / F;         // trajectories per warp
+  static constexpr int ACT = G * F;        // active lanes
+  static constexpr unsigned AMASK = ACT == 32 ? 0xffffffffu : ((1u << ACT) - 1u);
+  static constexpr int ND = F / 2 + 1;     // Hessian entries (a, (a+d)%F), d = 0..ND-1, computed by lane a
+  static constexpr int NR = (F - 1) / 2;   // cubic-gradient terms received from lanes a-d
+  static constexpr int FP = (F + 1) & ~1;  // F padded to even (16-byte alignment of the slots)
+  static constexpr int NH = F * ND;
+  static constexpr int NHP = (NH + 1) & ~1;
+  static constexpr int WS = FP + NHP + 2 * F;  // doubles of scratch per group: qs, Hs, red
+  // packed coefficient block
+  static constexpr int C3 = 0;                  // [ND][F][F]  (d, k, a) = Phi~[a][(a+d)%F][k]
+  static constexpr int C4U = C3 + ND * F * F;   // [F][F]      (j, a) = P~[a][j]
+  static constexpr int C4D = C4U + F * F;       // [ND][F]     (d, a) = P~[a][(a+d)%F]
+  static constexpr int W2 = C4D + ND * F;       // [F]         omega_a^2 / gamma_a
+  static constexpr int NCOEF_QFF = W2 + F;
+  static constexpr int NCOEF_MORSE = 3 * F;     // D[F], a~[F], Qe[F]
+  static constexpr int NCOEF = NCOEF_QFF > NCOEF_MORSE ? NCOEF_QFF : NCOEF_MORSE;
+  static constexpr int NCOEFP = (NCOEF + 1) & ~1;
+};
+
+// ---- a1: potential, own gradient component, ND Hessian entries (reduced coordinates) --------------
+// QFF (BASELINE.json configs 2-5, stand-in for the fitted surfaces of PAPER.md:157):
+//   H3_ab = sum_k Phi_abk Q_k,  g3_a = 1/2 sum_b H3_ab Q_b,  u_a = sum_j P_aj Q_j^2,
+//   g4_a = Q_a (u_a/2 - P_aa Q_a^2/3),  H4_aa = u_a/2,  H4_ab = P_ab Q_a Q_b,
+//   V = sum_a Q_a (w_a^2 Q_a/2 + g3_a/3 + g4_a/4)   (Euler's theorem on the homogeneous parts).
+// Morse: y = exp(-a (Q - Q_e)), V = D (1-y)^2, g = 2 D a y (1-y), H = 2 D a^2 y (2y-1).
+// Writes the entries to Hs[d*F + a]; the caller reads them back after __syncwarp.
+template <int F, int KIND>
+__device__ __forceinline__ void pes_group(const double *__restrict__ cs, double *qs, double *Hs, int a, int gbase,
+                                          const int (&fwd)[Geo<F>::ND], const int (&bwd)[Geo<F>::ND], double Q,
+                                          double &g, double &Va, double (&Hent)[Geo<F>::ND]) {
+  using X = Geo<F>;
+  if (KIND == SC_IVR_PES_QFF) {
+    double q[F];
+    if (F > 1) {
+      qs[a] = Q;
+      __syncwarp(X::AMASK);
+#pragma unroll
+      for (int i = 0; i < F; i++) q[i] = qs[i];
+    } else {
+      q[0] = Q;
+    }
+    double qd[X::ND];
+    qd[0] = Q;
+#pragma unroll
+    for (int d = 1; d < X::ND; d++) qd[d] = qs[fwd[d]];
+    double u = 0.0;
+#pragma unroll
+    for (int j = 0; j < F; j++) u = fma(cs[X::C4U + j * F + a], q[j] * q[j], u);
+    double h3[X::ND];
+#pragma unroll
+    for (int d = 0; d < X::ND; d++) {
+      double s = 0.0;
+#pragma unroll
+      for (int k = 0; k < F; k++) s = fma(cs[X::C3 + (d * F + k) * F + a], q[k], s);
+      h3[d] = s;
+    }
+    double s3 = 0.0;
+#pragma unroll
+    for (int d = 0; d < X::ND; d++) s3 = fma(h3[d], qd[d], s3);
+#pragma unroll
+    for (int d = 1; d <= X::NR; d++) s3 += __shfl_sync(X::AMASK, h3[d] * Q, gbase + bwd[d]);
+    const double w2 = cs[X::W2 + a];
+    const double paa = cs[X::C4D + a];
+    const double g3 = 0.5 * s3;
+    const double g4 = Q * (0.5 * u - (1.0 / 3.0) * paa * Q * Q);
+    g = fma(w2, Q, g3 + g4);
+    Va = Q * (0.5 * w2 * Q + (1.0 / 3.0) * g3 + 0.25 * g4);
+    Hent[0] = w2 + h3[0] + 0.5 * u;
+#pragma unroll
+    for (int d = 1; d < X::ND; d++) Hent[d] = fma(cs[X::C4D + d * F + a] * Q, qd[d], h3[d]);
+#pragma unroll
+    for (int d = 0; d < X::ND; d++) Hs[d * F + a] = Hent[d];
+  } else {
+    const double D = cs[a], at = cs[F + a], Qe = cs[2 * F + a];
+    const double y = exp(-at * (Q - Qe));
+    Va = D * (1.0 - y) * (1.0 - y);
+    g = 2.0 * D * at * y * (1.0 - y);
+    Hent[0] = 2.0 * D * at * at * y * (2.0 * y - 1.0);
+#pragma unroll
+    for (int d = 1; d < X::ND; d++) Hent[d] = 0.0;
+    Hs[a] = Hent[0];
+  }
+}
+
+// ---- a3 helper: HM1 = H dQ1, HM2 = H dQ2 from the group's shared Hessian slot ------------------------
+template <int F, int KIND>
+__device__ __forceinline__ void hessian_times_tangent(const double *Hs, const double (&dQ1)[F], const double (&dQ2)[F],
+                                                      double (&HM1)[F], double (&HM2)[F]) {
+  using X = Geo<F>;
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    const double h = Hs[i];
+    HM1[i] = h * dQ1[i];
+    HM2[i] = h * dQ2[i];
+  }
+  if (KIND == SC_IVR_PES_QFF) {
+#pragma unroll
+    for (int d = 1; d < X::ND; d++) {
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        if (F % 2 == 0 && d == F / 2 && i >= F / 2) continue;  // pair (i, i+F/2) already taken from lane i-F/2
+        const int l = (i + d) % F;
+        const double h = Hs[d * F + i];
+        HM1[i] = fma(h, dQ1[l], HM1[i]);
+        HM1[l] = fma(h, dQ1[i], HM1[l]);
+        HM2[i] = fma(h, dQ2[l], HM2[i]);
+        HM2[l] = fma(h, dQ2[i], HM2[l]);
+      }
+    }
+  }
+}
+
+// ---- a5: det of the F x F complex matrix whose column a is on lane a (Eq. 5) -------------
+// Elimination of rows k = 0..F-1 by column operations; the pivot for row k is the not-yet-used column with
+// the largest |A[k][.]| (REDUX over the group's lanes on the high word of |.|^2, lane id in the low bits).
+// det = sign(permutation) * product of pivots; the sign is the parity of the inversions of the pick order.
+template <int F>
+__device__ __forceinline__ void det_columns_complex(double (&Are)[F], double (&Aim)[F], int gbase, int a,
+                                                    unsigned gmask, double &Dre, double &Dim) {
+  using X = Geo<F>;
+  if (F == 1) {
+    Dre = Are[0];
+    Dim = Aim[0];
+    return;
+  }
+  unsigned umask = (1u << F) - 1u;
+  bool used = false;
+  unsigned par = 0;
+  double dre = 1.0, dim = 0.0;
+#pragma unroll
+  for (int k = 0; k < F; k++) {
+    const double mag = fma(Are[k], Are[k], Aim[k] * Aim[k]);
+    const unsigned key = used ? 0u : ((((unsigned)__double2hiint(mag)) & 0xFFFFFFE0u) | (unsigned)a) + 32u;
+    const unsigned best = __reduce_max_sync(gmask, key);
+    const int srcg = (int)((best - 32u) & 31u);
+    const int src = gbase + srcg;
+    par ^= __popc(umask & ((1u << srcg) - 1u));
+    umask &= ~(1u << srcg);
+    double pr[F], pi[F];
+#pragma unroll
+    for (int i = k; i < F; i++) {
+      pr[i] = __shfl_sync(X::AMASK, Are[i], src);
+      pi[i] = __shfl_sync(X::AMASK, Aim[i], src);
+    }
+    const double t = dre * pr[k] - dim * pi[k];
+    dim = fma(dre, pi[k], dim * pr[k]);
+    dre = t;
+    if (k < F - 1) {
+      const double rn = fast_rcp(fma(pr[k], pr[k], pi[k] * pi[k]));
+      const double ir = pr[k] * rn, ii = -pi[k] * rn;
+      const double mr = Are[k] * ir - Aim[k] * ii;
+      const double mi = fma(Are[k], ii, Aim[k] * ir);
+#pragma unroll
+      for (int i = k + 1; i < F; i++) {
+        Are[i] = fma(-mr, pr[i], fma(mi, pi[i], Are[i]));
+        Aim[i] = fma(-mr, pi[i], fma(-mi, pr[i], Aim[i]));
+      }
+    }
+    if (a == srcg) used = true;
+  }
+  if (par & 1u) {
+    dre = -dre;
+    dim = -dim;
+  }
+  Dre = dre;
+  Dim = dim;
+}
+
+// ---- a7: det of the 2F x 2F monodromy matrix; lane a holds columns a (in C[0..2F)) and F+a (C[2F..4F)) -----
+// Same column-pivoted elimination, two local columns per lane.  Reads its input from local memory so
+// that the caller's register state is not duplicated.
+template <int F>
+__device__ __noinline__ double det_columns_real2(const double *C, int gbase, int a, unsigned gmask) {
+  using X = Geo<F>;
+  constexpr int N = 2 * F;
+  double C1[N], C2[N];
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    C1[i] = C[i];
+    C2[i] = C[N + i];
+  }
+  bool used1 = false, used2 = false;
+  unsigned umask = (N >= 32) ? 0xffffffffu : ((1u << N) - 1u);
+  unsigned par = 0;
+  double det = 1.0;
+#pragma unroll
+  for (int k = 0; k < N; k++) {
+    const double m1 = used1 ? -1.0 : fabs(C1[k]);
+    const double m2 = used2 ? -1.0 : fabs(C2[k]);
+    const bool sel = m2 > m1;
+    const double m = sel ? m2 : m1;
+    const unsigned col_mine = (unsigned)(sel ? F + a : a);
+    const unsigned key = (m < 0.0) ? 0u : ((((unsigned)__double2hiint(m)) & 0xFFFFFFE0u) | col_mine) + 32u;
+    const unsigned best = (F == 1) ? key : __reduce_max_sync(gmask, key);
+    const int col = (int)((best - 32u) & 31u);
+    const bool ssel = col >= F;
+    const int srcg = ssel ? col - F : col;
+    const int src = gbase + srcg;
+    par ^= __popc(umask & ((1u << col) - 1u));
+    umask &= ~(1u << col);
+    double pv[N];
+#pragma unroll
+    for (int i = k; i < N; i++) {
+      const double v = ssel ? C2[i] : C1[i];
+      pv[i] = (F == 1) ? v : __shfl_sync(X::AMASK, v, src);
+    }
+    det *= pv[k];
+    if (k < N - 1) {
+      const double r = fast_rcp(pv[k]);
+      const double mm1 = C1[k] * r, mm2 = C2[k] * r;
+#pragma unroll
+      for (int i = k + 1; i < N; i++) {
+        C1[i] = fma(-mm1, pv[i], C1[i]);
+        C2[i] = fma(-mm2, pv[i], C2[i]);
+      }
+    }
+    if (a == srcg) {
+      if (ssel) used2 = true; else used1 = true;
+    }
+  }
+  return (par & 1u) ? -det : det;
+}
+
+template <int F, int KIND>
+__global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ PropParams P) {
+  using X = Geo<F>;
+  extern __shared__ double smem[];
+  double *cs = smem;
+  {
+    const int nco = (KIND == SC_IVR_PES_QFF) ? X::NCOEF_QFF : X::NCOEF_MORSE;
+    for (int i = threadIdx.x; i < nco; i += kThreads) cs[i] = P.coef[i];
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane >= X::ACT) return;
+  const int g = lane / F, a = lane - g * F, gbase = g * F;
+  const unsigned gmask = ((F == 32 ? 0u : (1u << F)) - 1u) << gbase;
+  double *ws = smem + X::NCOEFP + (warp * X::G + g) * X::WS;
+  double *qs = ws, *Hs = ws + X::FP;
+  double2 *red = reinterpret_cast<double2 *>(ws + X::FP + X::NHP);
+
+  const long long jj = (long long)blockIdx.x * (kThreads / 32 * X::G) + warp * X::G + g;
+  const bool valid = jj < P.nb;
+  const long long jl = valid ? jj : P.nb - 1;  // tail groups recompute the last trajectory and store nothing
+  const long long jg = P.j0 + jl;
+
+  int fwd[X::ND], bwd[X::ND];
+#pragma unroll
+  for (int d = 0; d < X::ND; d++) {
+    fwd[d] = (a + d) % F;
+    bwd[d] = (a - d + F) % F;
+  }
+  const double sg_a = P.sg[a], isg_a = P.isg[a], mu_a = P.mu[a];
+  const double Peq_a = P.Peq[a], Qeq_a = P.Qeq[a];
+
+  double Pm = P.p0q0[(long long)a * P.stride + jg] * isg_a;
+  double Q = P.p0q0[(long long)(F + a) * P.stride + jg] * sg_a;
+  double Sa = 0.0;
+  double dP1[F], dQ1[F], dP2[F], dQ2[F], HM1[F], HM2[F];
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    dP1[i] = (i == a) ? 1.0 : 0.0;
+    dQ1[i] = 0.0;
+    dP2[i] = 0.0;
+    dQ2[i] = (i == a) ? 1.0 : 0.0;
+  }
+  double gq, Va, Hent[X::ND];
+  pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
+  __syncwarp(X::AMASK);
+  hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
+
+  bool good = true;
+  bool dirty = false;
+  int det_count = 0;  // steps until the next check
+  const int nsteps = P.nsteps;
+#pragma unroll 1
+  for (int c = 0;; c++) {
+    // a5 (Eq. 5, R2): column a of 2K in reduced coordinates, then its determinant
+    double Dre, Dim;
+    {
+      double Are[F], Aim[F];
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        Are[i] = dQ2[i] + dP1[i];
+        Aim[i] = dP2[i] - dQ1[i];
+      }
+      det_columns_complex<F>(Are, Aim, gbase, a, gmask, Dre, Dim);
+    }
+    // a6 (Eq. 3): per-mode share of ln<chi|pq>; a8 input record
+    if (P.raw != nullptr) {
+      const double dq = Qeq_a - Q, dp = Peq_a - Pm;
+      const double oa = -0.25 * fma(dq, dq, dp * dp);
+      const double ob = 0.5 * (Peq_a + Pm) * dq;
+      if (F > 1) {
+        red[a] = make_double2(oa, Sa + ob);
+        __syncwarp(X::AMASK);
+        if (a == 0) {
+          double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+          for (int i = 0; i < F; i++) {
+            const double2 v = red[i];
+            s0 += v.x;
+            s1 += v.y;
+          }
+          if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre, Dim);
+        }
+      } else {
+        if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(oa, Sa + ob, Dre, Dim);
+      }
+    }
+    // a7: |det M - 1| <= tol and finite, every det_stride steps and at the end
+    if (det_count == 0 || c == nsteps) {
+      double buf[4 * F];
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        buf[i] = dP1[i];
+        buf[F + i] = dQ1[i];
+        buf[2 * F + i] = dP2[i];
+        buf[3 * F + i] = dQ2[i];
+      }
+      const double dM = det_columns_real2<F>(buf, gbase, a, gmask);
+      const bool ok = (fabs(dM - 1.0) <= P.det_tol) && isfinite(Sa) && isfinite(Pm) && isfinite(Q);
+      good = good && ok;
+      det_count = P.det_stride;
+    }
+    det_count--;
+    if (c == nsteps) break;
+    // a2-a4 (R10, R11): stages "kick b_i then drift a_i"; the PES is re-evaluated only after q moved
+#pragma unroll 1
+    for (int st = 0; st < P.nstages; st++) {
+      if (dirty) {
+        pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
+        __syncwarp(X::AMASK);
+        hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
+        dirty = false;
+      }
+      const double bdt = P.kick[st];
+      Sa = fma(-bdt, Va, Sa);
+      Pm = fma(-bdt, gq, Pm);
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        dP1[i] = fma(-bdt, HM1[i], dP1[i]);
+        dP2[i] = fma(-bdt, HM2[i], dP2[i]);
+      }
+      const double adt = P.drift[st];
+      if (adt != 0.0) {
+        Sa = fma(0.5 * adt * mu_a, Pm * Pm, Sa);
+        Q = fma(adt * mu_a, Pm, Q);
+#pragma unroll
+        for (int i = 0; i < F; i++) {
+          const double am = adt * P.mu[i];
+          dQ1[i] = fma(am, dP1[i], dQ1[i]);
+          dQ2[i] = fma(am, dP2[i], dQ2[i]);
+        }
+        dirty = true;
+      }
+    }
+  }
+
+  // outputs
+  const unsigned bal = __ballot_sync(X::AMASK, good);
+  const bool group_good = ((bal & gmask) == gmask);
+  double Stot = Sa;
+  if (F > 1) {
+    Stot = 0.0;
+#pragma unroll
+    for (int i = 0; i < F; i++) Stot += __shfl_sync(X::AMASK, Sa, gbase + i);
+  }
+  if (!valid) return;
+  if (P.good != nullptr && a == 0) P.good[jj] = group_good ? 1 : 0;
+  if (P.S_out != nullptr && a == 0) P.S_out[jg] = Stot;
+  if (P.pq_out != nullptr) {
+    P.pq_out[(long long)a * P.stride + jg] = Pm * sg_a;
+    P.pq_out[(long long)(F + a) * P.stride + jg] = Q * isg_a;
+  }
+  if (P.M_out != nullptr) {
+    // M_xy[i][a], reduced -> caller's units: p = sg P, q = Q / sg
+#pragma unroll
+    for (int i = 0; i < F; i++) {
+      const double si = P.sg[i], ii = P.isg[i];
+      const long long e = ((long long)i * F + a) * P.stride + jg;
+      const long long blk = (long long)F * F * P.stride;
+      P.M_out[0 * blk + e] = dP1[i] * si * isg_a;
+      P.M_out[1 * blk + e] = dP2[i] * si * sg_a;
+      P.M_out[2 * blk + e] = dQ1[i] * ii * isg_a;
+      P.M_out[3 * blk + e] = dQ2[i] * ii * sg_a;
+    }
+  }
+}
+
+// ---- debug kernel for a1: same pes_group, caller's units out -----------------------------------------------
+template <int F, int KIND>
+__global__ void __launch_bounds__(kThreads) k_eval_pes(const double *__restrict__ coef, const double *__restrict__ sgv,
+                                                       const double *__restrict__ q, long long n, double *V, double *gout,
+                                                       double *H) {
+  using X = Geo<F>;
+  extern __shared__ double smem[];
+  double *cs = smem;
+  {
+    const int nco = (KIND == SC_IVR_PES_QFF) ? X::NCOEF_QFF : X::NCOEF_MORSE;
+    for (int i = threadIdx.x; i < nco; i += kThreads) cs[i] = coef[i];
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane >= X::ACT) return;
+  const int g = lane / F, a = lane - g * F, gbase = g * F;
+  double *ws = smem + X::NCOEFP + (warp * X::G + g) * X::WS;
+  double *qs = ws, *Hs = ws + X::FP;
+  const long long jj = (long long)blockIdx.x * (kThreads / 32 * X::G) + warp * X::G + g;
+  const bool valid = jj < n;
+  const long long jl = valid ? jj : n - 1;
+  int fwd[X::ND], bwd[X::ND];
+#pragma unroll
+  for (int d = 0; d < X::ND; d++) {
+    fwd[d] = (a + d) % F;
+    bwd[d] = (a - d + F) % F;
+  }
+  const double sg_a = sgv[a];
+  const double Q = q[(long long)a * n + jl] * sg_a;
+  double gq, Va, Hent[X::ND];
+  pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
+  double Vt = 0.0;
+#pragma unroll
+  for (int i = 0; i < F; i++) Vt += __shfl_sync(X::AMASK, Va, gbase + i);
+  if (!valid) return;
+  if (a == 0) V[jl] = Vt;
+  gout[(long long)a * n + jl] = gq * sg_a;
+  if (KIND != SC_IVR_PES_QFF) {
+    for (int b = 0; b < F; b++) H[((long long)a * F + b) * n + jl] = (b == a) ? Hent[0] * sg_a * sg_a : 0.0;
+  } else {
+#pragma unroll
+    for (int d = 0; d < X::ND; d++) {
+      const int b = fwd[d];
+      const double h = Hent[d] * sg_a * sgv[b];
+      H[((long long)a * F + b) * n + jl] = h;
+      H[((long long)b * F + a) * n + jl] = h;
+    }
+  }
+}
+
+template <int F>
+size_t smem_bytes() {
+  return sizeof(double) * (Geo<F>::NCOEFP + (kThreads / 32) * Geo<F>::G * Geo<F>::WS);
+}
+
+template <int F, int KIND>
+cudaError_t launch_prop(const PropParams &P, cudaStream_t st) {
+  const int tpb = (kThreads / 32) * Geo<F>::G;
+  const long long blocks = (P.nb + tpb - 1) / tpb;
+  k_propagate<F, KIND><<<(unsigned)blocks, kThreads, smem_bytes<F>(), st>>>(P);
+  return cudaGetLastError();
+}
+
+template <int F, int KIND>
+cudaError_t launch_pes(const double *coef, const double *sg, const double *q, long long n, double *V, double *g, double *H,
+                       cudaStream_t st) {
+  const int tpb = (kThreads / 32) * Geo<F>::G;
+  const long long blocks = (n + tpb - 1) / tpb;
+  k_eval_pes<F, KIND><<<(unsigned)blocks, kThreads, smem_bytes<F>(), st>>>(coef, sg, q, n, V, g, H);
+  return cudaGetLastError();
+}
+
+template <int F, int KIND>
+int occupancy() {
+  int nb = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_propagate<F, KIND>, kThreads, smem_bytes<F>()) != cudaSuccess) nb = 1;
+  return nb < 1 ? 1 : nb;
+}
+
+}  // namespace
+
+#define SCI_FOR_EACH_F(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
+
+int sci_prop_traj_per_block(int F) { return (kThreads / 32) * (32 / F); }
+
+int sci_prop_blocks_per_sm(int F, int kind) {
+  const bool qff = kind == SC_IVR_PES_QFF;
+  switch (F) {
+#define X(f) case f: return qff ? occupancy<f, SC_IVR_PES_QFF>() : occupancy<f, SC_IVR_PES_MORSE_UNCOUPLED>();
+    SCI_FOR_EACH_F(X)
+#undef X
+  }
+  return 1;
+}
+
+cudaError_t sci_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st) {
+  const bool qff = kind == SC_IVR_PES_QFF;
+  switch (F) {
+#define X(f) case f: return qff ? launch_prop<f, SC_IVR_PES_QFF>(P, st) : launch_prop<f, SC_IVR_PES_MORSE_UNCOUPLED>(P, st);
+    SCI_FOR_EACH_F(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t sci_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q, long long n,
+                                double *V, double *g, double *H, cudaStream_t st) {
+  const bool qff = kind == SC_IVR_PES_QFF;
+  switch (F) {
+#define X(f) case f: return qff ? launch_pes<f, SC_IVR_PES_QFF>(coef, sg, q, n, V, g, H, st) \
+                                : launch_pes<f, SC_IVR_PES_MORSE_UNCOUPLED>(coef, sg, q, n, V, g, H, st);
+    SCI_FOR_EACH_F(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+
+// Host: reduce the caller's coefficients to the kernel's packed block (layout in Geo<F>).
+//   Phi~_ijk = Phi_ijk / sqrt(g_i g_j g_k),  P~_ij = Phi_iijj / (g_i g_j),  w~_a^2 = w_a^2 / g_a   (QFF)
+//   a~ = a / sqrt(g),  Q_e = sqrt(g) q_e                                                           (Morse)
+size_t sci_pack_coeffs(int F, int kind, const double *c, const double *gamma, double *out) {
+  const int ND = F / 2 + 1;
+  if (kind != SC_IVR_PES_QFF) {
+    const size_t n = 3 * (size_t)F;
+    if (!out) return n;
+    for (int a = 0; a < F; a++) {
+      const double sg = sqrt(gamma[a]);
+      out[a] = c[4 * a];
+      out[F + a] = c[4 * a + 1] / sg;
+      out[2 * F + a] = c[4 * a + 2] * sg;
+    }
+    return n;
+  }
+  const int C3 = 0, C4U = C3 + ND * F * F, C4D = C4U + F * F, W2 = C4D + ND * F;
+  const size_t n = (size_t)W2 + F;
+  if (!out) return n;
+  // unpack the symmetric tensors
+  double *phi = new double[(size_t)F * F * F];
+  double *pq = new double[(size_t)F * F];
+  const double *cub = c + F;
+  size_t m = 0;
+  for (int i = 0; i < F; i++)
+    for (int j = i; j < F; j++)
+      for (int k = j; k < F; k++) {
+        const double v = cub[m++] / sqrt(gamma[i] * gamma[j] * gamma[k]);
+        const int p[6][3] = {{i, j, k}, {i, k, j}, {j, i, k}, {j, k, i}, {k, i, j}, {k, j, i}};
+        for (auto &t : p) phi[((size_t)t[0] * F + t[1]) * F + t[2]] = v;
+      }
+  const double *qua = cub + m;
+  m = 0;
+  for (int i = 0; i < F; i++)
+    for (int j = i; j < F; j++) {
+      const double v = qua[m++] / (gamma[i] * gamma[j]);
+      pq[i * F + j] = pq[j * F + i] = v;
+    }
+  for (int d = 0; d < ND; d++)
+    for (int k = 0; k < F; k++)
+      for (int a = 0; a < F; a++) out[C3 + (d * F + k) * F + a] = phi[((size_t)a * F + (a + d) % F) * F + k];
+  for (int j = 0; j < F; j++)
+    for (int a = 0; a < F; a++) out[C4U + j * F + a] = pq[a * F + j];
+  for (int d = 0; d < ND; d++)
+    for (int a = 0; a < F; a++) out[C4D + d * F + a] = pq[a * F + (a + d) % F];
+  for (int a = 0; a < F; a++) out[W2 + a] = c[a] * c[a] / gamma[a];
+  delete[] phi;
+  delete[] pq;
+  return n;
+}

@@ -1,0 +1,259 @@
+"""GPU parity: the CUDA path (through the C ABI, paper_1312_4698_b200.binding) against the CPU oracle on
+the same seeded inputs.  Tolerances are BASELINE.json's north star: (p, q, S) to 1e-10 norm-relative after
+1000 steps (R20), I(E) to 1e-8 of its maximum with identical peak bins (R19).
+"""
+import numpy as np
+import pytest
+
+from paper_1312_4698_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_STATE = 1e-10
+TOL_I = 1e-8
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1312_4698_b200 import binding
+    binding.lib()  # fails loudly if the extension is missing
+    return binding
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _relnorm(x, ref):
+    return np.max(np.abs(x - ref)) / max(np.max(np.abs(ref)), 1e-300)
+
+
+def _workloads_small():
+    return [
+        inputs.make_config(1, ntraj=131, nsteps=1000, k=64),
+        inputs.make_config(2, ntraj=203, nsteps=1000, k=64),
+        inputs.make_config(3, ntraj=77, nsteps=1000, k=64),
+        inputs.make_config(4, ntraj=100, nsteps=1000, k=64),
+        inputs.make_random_qff(2, 37, 1000, 64, seed=5),
+        inputs.make_random_qff(4, 41, 1000, 64, seed=6),
+        inputs.make_random_qff(5, 29, 1000, 64, seed=7),
+        inputs.make_random_qff(7, 23, 1000, 64, seed=8),
+        inputs.make_random_qff(8, 19, 1000, 64, seed=9),
+        inputs.make_random_qff(12, 9, 500, 64, seed=10),
+        inputs.make_uncoupled_morse(3, 50, 1000, 64),
+    ]
+
+
+@pytest.mark.parametrize("w", _workloads_small(), ids=lambda w: w.name)
+def test_pes_parity(torch_cuda, B, oracle, w):
+    """a1: V, g, H of the device PES code vs the oracle, at the workload's initial positions (ragged n)."""
+    torch = torch_cuda
+    q = np.ascontiguousarray(w.p0q0[w.F:, :])
+    ctx = B.ScIvr.from_workload(w)
+    V, g, H = ctx.eval_pes(_dev(torch, q))
+    Vo, go, Ho = oracle.eval_pes(w.F, w.pes_kind, w.pes_coeffs, q)
+    assert _relnorm(V.cpu().numpy(), Vo) < 1e-13
+    assert _relnorm(g.cpu().numpy(), go) < 1e-13
+    assert _relnorm(H.cpu().numpy(), Ho) < 1e-13
+
+
+@pytest.mark.parametrize("w", _workloads_small(), ids=lambda w: w.name)
+def test_propagate_parity_1000_steps(torch_cuda, B, oracle, w):
+    """a2-a7: (p, q, S) to 1e-10 norm-relative after 1000 steps; M, theta, flags and z alongside."""
+    torch = torch_cuda
+    ctx = B.ScIvr.from_workload(w)
+    o = ctx.propagate(_dev(torch, w.p0q0), w.nsteps, chi=w.chi, want_z=True)
+    r = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, w.chi, want_z=True)
+    F = w.F
+    pq = o["pq"].cpu().numpy()
+    assert _relnorm(pq[:F], r["pq"][:F]) < TOL_STATE
+    assert _relnorm(pq[F:], r["pq"][F:]) < TOL_STATE
+    assert _relnorm(o["S"].cpu().numpy(), r["S"]) < TOL_STATE
+    M = o["M"].cpu().numpy()
+    for b in range(4):
+        assert _relnorm(M[b], r["M"][b]) < 1e-9
+    assert np.max(np.abs(o["theta"].cpu().numpy() - r["theta"])) < 1e-8
+    assert np.array_equal(o["good"].cpu().numpy(), r["good"])
+    z = o["z"].cpu().numpy().T  # [n][c]
+    assert np.max(np.abs(z - r["z"])) < 1e-9
+
+
+def test_propagate_fourth_order_and_stride(torch_cuda, B, oracle):
+    """The 4-stage scheme and det_stride > 1 follow the oracle too."""
+    torch = torch_cuda
+    w = inputs.make_config(2, ntraj=67, nsteps=300, k=8)
+    ctx = B.ScIvr.from_workload(w, integrator=1, det_stride=7)
+    o = ctx.propagate(_dev(torch, w.p0q0), 300, chi=w.chi)
+    r = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, 300, w.p0q0, w.chi, integrator=1, det_stride=7)
+    assert _relnorm(o["pq"].cpu().numpy(), r["pq"]) < TOL_STATE
+    assert _relnorm(o["S"].cpu().numpy(), r["S"]) < TOL_STATE
+    assert np.max(np.abs(o["theta"].cpu().numpy() - r["theta"])) < 1e-8
+    assert np.array_equal(o["good"].cpu().numpy(), r["good"])
+
+
+def test_propagate_zero_steps(torch_cuda, B):
+    """P0: M = I, S = 0, theta = 0, z_0 = <chi|p0 q0>; started at chi, z_0 = 1."""
+    torch = torch_cuda
+    w = inputs.make_config(4, ntraj=5, nsteps=10, k=8)
+    p0q0 = w.p0q0.copy()
+    p0q0[:, 0] = w.chi
+    ctx = B.ScIvr.from_workload(w)
+    o = ctx.propagate(_dev(torch, p0q0), 0, chi=w.chi, want_z=True)
+    assert np.allclose(o["pq"].cpu().numpy(), p0q0, rtol=1e-15, atol=0)
+    assert np.all(o["S"].cpu().numpy() == 0) and np.all(o["theta"].cpu().numpy() == 0)
+    M = o["M"].cpu().numpy()
+    eye = np.eye(w.F)
+    for j in range(5):
+        assert np.allclose(M[0, :, :, j], eye, atol=1e-15) and np.allclose(M[3, :, :, j], eye, atol=1e-15)
+        assert not M[1, :, :, j].any() and not M[2, :, :, j].any()
+    z0 = o["z"].cpu().numpy()[0]
+    assert abs(z0[0] - 1.0) < 1e-14 and np.all(np.abs(z0[1:]) < 1.0)
+
+
+def test_fourier_parity(torch_cuda, B, oracle):
+    """a8 alone: the production Fourier kernel vs the definition (one cexp per term), ragged sizes."""
+    torch = torch_cuda
+    rng = np.random.default_rng(3)
+    nsteps, n, k = 333, 150, 70
+    w = inputs.make_config(1, ntraj=2, nsteps=nsteps, k=k)
+    z = (rng.standard_normal((n, nsteps + 1)) + 1j * rng.standard_normal((n, nsteps + 1))) * 0.3
+    ctx = B.ScIvr.from_workload(w)
+    A = ctx.fourier(_dev(torch, z.T.copy()), w.E).cpu().numpy()
+    Ao = oracle.fourier(z, w.dt, w.E, mode=0)
+    assert np.max(np.abs(A - Ao)) < 1e-11 * np.max(np.abs(Ao))
+
+
+def _run_both(torch, B, oracle, w, **kw):
+    ctx = B.ScIvr.from_workload(w, **kw)
+    I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
+    Io, ngo, rco = oracle.run_workload(w, **kw)
+    return I.cpu().numpy(), ng, rc, Io, ngo, rco
+
+
+def _assert_spectrum(oracle, I, Io):
+    mx = Io.max()
+    assert mx > 0 and np.all(I >= 0)
+    assert np.max(np.abs(I - Io)) <= TOL_I * mx
+    pk, pko = oracle.find_peaks(I), oracle.find_peaks(Io)
+    if not np.array_equal(pk, pko):  # R19: only bins whose margin is below 1e-7 max may legitimately flip
+        for i in set(pk.tolist()) ^ set(pko.tolist()):
+            margin = min(abs(Io[i] - Io[i - 1]), abs(Io[i] - Io[i + 1]), abs(Io[i] - 1e-3 * mx))
+            assert margin < 1e-7 * mx, f"peak bin {i} differs with margin {margin / mx:.2e}"
+
+
+def test_run_parity_config1_full(torch_cuda, B, oracle):
+    """Config 1 at its full size: 1024 trajectories, 3000 steps, 2000 energies."""
+    w = inputs.make_config(1)
+    I, ng, rc, Io, ngo, rco = _run_both(torch_cuda, B, oracle, w)
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I, Io)
+
+
+@pytest.mark.parametrize("cfg,ntraj", [(2, 300), (3, 200), (4, 150)])
+def test_run_parity_configs_full_time_and_energy_grid(torch_cuda, B, oracle, cfg, ntraj):
+    """Configs 2-4 with their full time and energy grids (4000 steps, 4000 energies) on a trajectory
+    prefix the oracle finishes in seconds; ragged against every tile size."""
+    w = inputs.make_config(cfg, ntraj=ntraj)
+    I, ng, rc, Io, ngo, rco = _run_both(torch_cuda, B, oracle, w)
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I, Io)
+
+
+def test_run_weights_poison_and_rejection(torch_cuda, B, oracle):
+    """P11 on the GPU: explicit weights; a NaN trajectory drops out (n_good - 1) without touching the rest;
+    a tolerance nobody meets gives ENOGOOD and a zero spectrum (R18)."""
+    torch = torch_cuda
+    w = inputs.make_config(2, ntraj=90, nsteps=400, k=300)
+    rng = np.random.default_rng(1)
+    wt = rng.uniform(0.5, 1.5, w.ntraj)
+    ctx = B.ScIvr.from_workload(w)
+    I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E, weights=_dev(torch, wt))
+    Io, ngo, _ = oracle.run(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, w.chi, w.E, weights=wt)
+    assert ng == ngo == w.ntraj
+    _assert_spectrum(oracle, I.cpu().numpy(), Io)
+    p = w.p0q0.copy()
+    p[1, 17] = np.nan
+    Ip, ngp, _ = ctx.run(_dev(torch, p), w.chi, w.E)
+    keep = np.ones(w.ntraj, bool)
+    keep[17] = False
+    Ik, ngk, _ = oracle.run(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, np.ascontiguousarray(w.p0q0[:, keep]), w.chi, w.E)
+    assert ngp == ngk == w.ntraj - 1
+    _assert_spectrum(oracle, Ip.cpu().numpy(), Ik)
+    strict = B.ScIvr.from_workload(w, det_tol=1e-300)
+    Iz, ngz, rcz = strict.run(_dev(torch, w.p0q0), w.chi, w.E)
+    assert rcz == B.ENOGOOD and ngz == 0 and not Iz.cpu().numpy().any()
+
+
+def test_run_batches_deterministic_and_single_trajectory(torch_cuda, B, oracle):
+    """Several batches (small workspace) agree with one batch to round-off; repeated runs are bitwise equal
+    (fixed reduction order); ntraj = 1 works."""
+    torch = torch_cuda
+    w = inputs.make_config(3, ntraj=3000, nsteps=200, k=130)
+    ctx = B.ScIvr.from_workload(w)
+    d = _dev(torch, w.p0q0)
+    I1, ng1, _ = ctx.run(d, w.chi, w.E)
+    I2, ng2, _ = ctx.run(d, w.chi, w.E)
+    assert torch.equal(I1, I2) and ng1 == ng2 == 3000
+    mb = ctx.min_batch()
+    if mb < 3000:
+        Ib, ngb, _ = ctx.run(d, w.chi, w.E, max_batch=mb)
+        assert ngb == 3000
+        assert np.max(np.abs(Ib.cpu().numpy() - I1.cpu().numpy())) <= 1e-13 * I1.max().item()
+    w1 = w.prefix(1)
+    Is, ngs, _ = ctx.run(_dev(torch, w1.p0q0), w.chi, w.E)
+    Io, ngo, _ = oracle.run_workload(w1)
+    assert ngs == ngo == 1
+    _assert_spectrum(oracle, Is.cpu().numpy(), Io)
+
+
+def test_run_host_matches_device_entry(torch_cuda, B):
+    torch = torch_cuda
+    w = inputs.make_config(2, ntraj=500, nsteps=300, k=200)
+    ctx = B.ScIvr.from_workload(w)
+    I, ng, _ = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
+    Ih, ngh, _ = ctx.run_host(w.p0q0, w.chi, w.E)
+    assert ngh == ng and np.array_equal(Ih, I.cpu().numpy())
+
+
+def test_error_paths(torch_cuda, B):
+    torch = torch_cuda
+    w = inputs.make_config(2, ntraj=64, nsteps=50, k=16)
+    with pytest.raises(B.ScIvrError) as e:
+        B.ScIvr(w.F, w.pes_kind, w.pes_coeffs[:-1], w.gamma, w.dt, w.nsteps)
+    assert e.value.status == B.EINVAL
+    with pytest.raises(B.ScIvrError) as e:
+        B.ScIvr(13, inputs.PES_QFF, np.zeros(13 + 455 + 91), np.ones(13), 1.0, 10)
+    assert e.value.status == B.EUNSUPPORTED
+    with pytest.raises(B.ScIvrError) as e:
+        B.ScIvr(w.F, w.pes_kind, w.pes_coeffs, -w.gamma, w.dt, w.nsteps)
+    assert e.value.status == B.EINVAL
+    ctx = B.ScIvr.from_workload(w)
+    with pytest.raises(B.ScIvrError) as e:
+        ctx.run(_dev(torch, w.p0q0), w.chi, w.E, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == B.EINVAL and "workspace" in str(e.value)
+
+
+def test_full_size_config4_sampled_trajectories(torch_cuda, B, oracle):
+    """Config 4 at BASELINE.json's full size, in the launch configuration bench.py times (one call, all 131072
+    trajectories, 4000 steps, 4000 energies).  Outputs the oracle can compute one by one: the weights select
+    24 sampled trajectories (weight 1, everything else 0), so I(E) n_good / n_sample is exactly the oracle's
+    spectrum of those 24 alone; n_good itself must be the full count."""
+    torch = torch_cuda
+    w = inputs.make_config(4)
+    rng = np.random.default_rng(99)
+    pick = np.sort(rng.choice(w.ntraj, 24, replace=False))
+    wt = np.zeros(w.ntraj)
+    wt[pick] = 1.0
+    ctx = B.ScIvr.from_workload(w)
+    I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E, weights=_dev(torch, wt))
+    assert rc == 0 and ng == w.ntraj
+    Io, ngo, _ = oracle.run(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, np.ascontiguousarray(w.p0q0[:, pick]), w.chi, w.E)
+    assert ngo == 24
+    _assert_spectrum(oracle, I.cpu().numpy() * (ng / 24.0), Io)
