@@ -1,0 +1,264 @@
+#!/usr/bin/env python
+"""bench.py - trajectory-steps/s of the whole TA-SC-IVR hot path (all SURVEY.md 8a rows) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--det-stride D] [--impl reference]
+
+A "step" is one sc_ivr_run over the whole workload: propagate (PES, symplectic step, monodromy, action,
+Herman-Kluk determinant, overlap, det M flag at every time step) -> z assembly -> Fourier sum -> |.|^2
+reduction -> I(E).  Default workload: BASELINE.json config 4 (CH4-like, F = 9, 131072 trajectories,
+4000 time steps, 4000 energies), the configuration the north star's target is quoted on.
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1312_4698_b200 import inputs  # noqa: E402
+
+METRIC = "FP64 trajectory-steps/sec (with monodromy+prefactor)"
+UNIT = "trajectory-steps/s"
+# FP64 roofline denominator: 148 SMs x 64 FP64 FMA lanes/SM/clk x 2 flop x 1.965 GHz.
+# The guides give no FP64 unit count; 64 lanes/SM/clk is what this library's own DFMA/DMMA probe
+# measures (37.2 TFLOP/s with mma.sync m8n8k4 f64 at 1965 MHz) - the probe value is reported beside it.
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the bench configuration,
+# from the ncu --set full capture summarised in profiles/ (None until captured).
+NCU_TRAFFIC_BYTES = {"propagate": None, "fourier": None}
+
+
+def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False):
+    """Algorithmic flop per trajectory-step (SURVEY.md 8d table, 1 FMA = 2 flop)."""
+    pes = 60 if morse else 2 * (F * F * (F + 1) // 2 + 2 * F * F + F * (F - 1) + 6 * F)
+    step = 16 * F + 6
+    mono = 2 * (2 * F ** 3 + 6 * F ** 2)
+    kmat = 6 * F * F
+    cdet = 8 * (F - 1) * F * (2 * F - 1) // 6 + 6 * F * (F - 1) // 2 + 16 * F
+    transc = 150
+    a_total = pes + step + mono + kmat + cdet + transc
+    n = 2 * F
+    check = 2 * ((n - 1) * n * (2 * n - 1) // 6) + n * (n - 1) // 2 + 12 * n
+    if det_every_step:
+        a_total += check
+    return dict(propagate=a_total, fourier=8 * k)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_ev = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_ev.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.splitlines()[0].split(",")])
+            except Exception:
+                pass
+            self._stop_ev.wait(0.2)
+
+    def stop(self):
+        self._stop_ev.set()
+        self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=reasons,
+                    samples=len(sm))
+
+
+def cpu_oracle_sample(w, ntraj_sample: int, det_stride: int):
+    """The oracle as it stands, on the first ntraj_sample trajectories of the workload (full time and energy grid)."""
+    from oracle import capi
+    ws = w.prefix(min(ntraj_sample, w.ntraj))
+    t0 = time.perf_counter()
+    capi.run_workload(ws, det_stride=det_stride)
+    dt = time.perf_counter() - t0
+    return dict(value=ws.ntraj * w.nsteps / dt, unit=UNIT, cores=capi.num_threads(), kind="oracle",
+                sample=f"first {ws.ntraj} trajectories of {w.name}, {w.nsteps} steps, {w.k} energies, det_stride={det_stride}: {dt:.1f} s"), dt
+
+
+def make_workload(config: int, rank: int, ntraj: int | None):
+    if rank == 0 and config != 5:
+        return inputs.make_config(config, ntraj=ntraj)
+    # rank r > 0 (weak scaling): block r of config 5's 2^20-row draw on config 4's surface, same size as rank 0's
+    n = ntraj or inputs._DEFAULTS[4 if config == 5 else config]["ntraj"]
+    full = inputs.make_config(5, ntraj=min((rank + 1) * n, 1 << 20))
+    w = full.prefix(full.ntraj)
+    w.p0q0 = np.ascontiguousarray(full.p0q0[:, full.ntraj - n:])
+    return w
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    w = make_workload(args.config, 0, args.ntraj)
+    times = []
+    for i in range(args.warmup + args.steps):
+        cb, dt = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
+        if i >= args.warmup:
+            times.append(dt)
+    n = min(args.ref_sample, w.ntraj)
+    val = n * w.nsteps / (sum(times) / len(times))
+    cb["value"] = val
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "F": w.F, "ntraj_sample": n, "nsteps": w.nsteps, "k": w.k, "det_stride": args.det_stride},
+        "cpu_baseline": cb, "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--ntraj", type=int, default=None)
+    ap.add_argument("--det-stride", type=int, default=1)
+    ap.add_argument("--ref-sample", type=int, default=1024)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1312_4698_b200 import binding as B
+    from paper_1312_4698_b200.sharding import combine_spectra
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    B.lib()
+
+    w = make_workload(args.config, rank, args.ntraj)
+    ctx = B.ScIvr.from_workload(w, det_stride=args.det_stride)
+    ctx.set_timing(True)
+    d_pq = torch.from_numpy(w.p0q0).cuda()
+    ws_bytes = ctx.workspace_bytes(w.ntraj, w.k) + ctx.host_staging_bytes(w.ntraj, w.k)
+    wsp = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
+    I_dev = torch.empty(w.k, dtype=torch.float64, device="cuda")
+    h_pq = torch.from_numpy(w.p0q0).pin_memory()
+    h_I = torch.empty(w.k, dtype=torch.float64).pin_memory()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        ctx.run(d_pq, w.chi, w.E, I_out=I_dev, workspace=wsp, want_n_good=False)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage = dict(propagate_ms=0.0, zassemble_ms=0.0, twiddle_ms=0.0, fourier_ms=0.0, reduce_ms=0.0)
+    launches = 0
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    t = ctx.last_timings()  # stage events of the LAST timed step (recorded on the run stream, no sync inside)
+    launches = t["launches"] * args.steps
+    for key in stage:
+        stage[key] = t[key]
+    # end to end through the C ABI with HOST buffers: H2D of p0q0, D2H of I(E) inside the timed region
+    barrier()
+    for _ in range(1):
+        ctx.run_host(h_pq, w.chi, w.E, I_out=h_I, workspace=wsp)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, ng_host, _ = ctx.run_host(h_pq, w.chi, w.E, I_out=h_I, workspace=wsp)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    clocks = sampler.stop()
+
+    tt = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        # the path's only exchange: k + 1 doubles (sharding.combine_spectra)
+        I_all, ng_all = combine_spectra(I_dev, ng_host)
+    ms, e2e_ms = tt[0].item(), tt[1].item()
+    units = w.ntraj * w.nsteps * args.steps * world
+    value = units / (ms * 1e-3)
+    e2e_value = units / (e2e_ms * 1e-3)
+
+    if rank == 0:
+        fm = flop_model(w.F, w.k, args.det_stride == 1, morse=(w.pes_kind != inputs.PES_QFF))
+        dom = "fourier" if stage["fourier_ms"] >= stage["propagate_ms"] else "propagate"
+        dom_ms = stage[dom + "_ms"]
+        flops_per_launch = fm[dom] * w.ntraj * w.nsteps  # one launch per run when the workload is a single batch
+        achieved = flops_per_launch / (dom_ms * 1e-3) / 1e12
+        other = "propagate" if dom == "fourier" else "fourier"
+        other_tf = fm[other] * w.ntraj * w.nsteps / (stage[other + "_ms"] * 1e-3) / 1e12
+        try:
+            probe = {"dfma_tflops": B.fp64_probe(0, 20000)[0] / 1e12, "dmma_tflops": B.fp64_probe(1, 20000)[0] / 1e12}
+        except Exception as ex:  # measurement helper only
+            probe = {"error": str(ex)}
+        cpu = None
+        if not args.no_cpu_baseline:
+            cpu, _ = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "F": w.F, "ntraj_per_gpu": w.ntraj, "nsteps": w.nsteps, "k": w.k, "dt": w.dt,
+                       "det_stride": args.det_stride, "integrator": "velocity-verlet",
+                       "l2": "working set per step (raw 32 B + z 16 B per trajectory-step) exceeds L2 by >100x; no flush needed",
+                       "parallelism": f"trajectory shards x{world}, one all-reduce of k+1 doubles" if world > 1 else "single GPU"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.p0q0.nbytes + w.E.nbytes),
+                    "d2h_bytes_per_step": int(w.k * 8 + 8)},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES[dom],
+                         "peak_source": "148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); this run's FP64 probes alongside",
+                         "flop_per_trajectory_step": fm[dom], "probe": probe,
+                         "other_kernel": {"kernel": "k_" + other, "achieved": other_tf, "frac": other_tf / FP64_PEAK_TFLOPS,
+                                          "flop_per_trajectory_step": fm[other]}},
+            "stage_ms_last_step": stage,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -106,17 +106,28 @@ struct StageTimer {
   sc_ivr_ctx *ctx;
   cudaStream_t st;
   bool on;
-  StageTimer(sc_ivr_ctx *c, cudaStream_t s) : ctx(c), st(s), on(c->timing != 0) {}
-  void begin() {
-    if (on) cudaEventRecord(ctx->ev[0], st);
+  StageTimer(sc_ivr_ctx *c, cudaStream_t s) : ctx(c), st(s), on(c->timing != 0) {
+    if (on) {
+      ctx->ev_used = 0;
+      ctx->ev_slot.clear();
+    }
   }
-  void end(int slot) {  // synchronising: only used when timing is switched on
+  void begin() {
     if (!on) return;
-    cudaEventRecord(ctx->ev[1], st);
-    cudaEventSynchronize(ctx->ev[1]);
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]);
-    ctx->tms[slot] += ms;
+    if (ctx->ev.size() < ctx->ev_used + 2) {
+      cudaEvent_t a = nullptr, b = nullptr;
+      cudaEventCreate(&a);
+      cudaEventCreate(&b);
+      ctx->ev.push_back(a);
+      ctx->ev.push_back(b);
+    }
+    cudaEventRecord(ctx->ev[ctx->ev_used], st);
+  }
+  void end(int slot) {
+    if (!on) return;
+    cudaEventRecord(ctx->ev[ctx->ev_used + 1], st);
+    ctx->ev_used += 2;
+    ctx->ev_slot.push_back(slot);
   }
 };
 
@@ -159,9 +170,8 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
     return fail(ctx, SC_IVR_ECUDA, "no CUDA device (%s): this library has no CPU fallback",
                 ce == cudaSuccess ? "device count 0" : cudaGetErrorString(ce));
 
-  ctx = new (std::nothrow) sc_ivr_ctx;
+  ctx = new (std::nothrow) sc_ivr_ctx();
   if (!ctx) return fail(nullptr, SC_IVR_ENOMEM, "out of host memory");
-  memset(ctx, 0, sizeof(*ctx));
   ctx->F = F;
   ctx->kind = (int)kind;
   ctx->nsteps = nsteps;
@@ -204,10 +214,6 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
       rc = fail(nullptr, SC_IVR_ECUDA, "coefficient upload: %s", cudaGetErrorString(ce));
       break;
     }
-    if (cudaEventCreate(&ctx->ev[0]) != cudaSuccess || cudaEventCreate(&ctx->ev[1]) != cudaSuccess) {
-      rc = fail(nullptr, SC_IVR_ECUDA, "event creation failed");
-      break;
-    }
     ctx->wave = (long long)ctx->sm_count * sci_prop_blocks_per_sm(F, (int)kind) * sci_prop_traj_per_block(F);
   } while (0);
   if (rc != SC_IVR_OK) {
@@ -221,8 +227,8 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
 void sc_ivr_destroy(sc_ivr_ctx *ctx) {
   if (!ctx) return;
   if (ctx->d_coef) cudaFree(ctx->d_coef);
-  if (ctx->ev[0]) cudaEventDestroy(ctx->ev[0]);
-  if (ctx->ev[1]) cudaEventDestroy(ctx->ev[1]);
+  for (cudaEvent_t e : ctx->ev)
+    if (e) cudaEventDestroy(e);
   delete ctx;
 }
 
@@ -245,6 +251,13 @@ void sc_ivr_set_timing(sc_ivr_ctx *ctx, int on) {
 
 sc_ivr_status sc_ivr_last_timings(sc_ivr_ctx *ctx, double out[6]) {
   if (!ctx || !out) return SC_IVR_EINVAL;
+  if (ctx->ev_used >= 2) CU(cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
+  for (int i = 0; i < 5; i++) ctx->tms[i] = 0.0;
+  for (size_t p = 0; p < ctx->ev_slot.size(); p++) {
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, ctx->ev[2 * p], ctx->ev[2 * p + 1]));
+    ctx->tms[ctx->ev_slot[p]] += ms;
+  }
   for (int i = 0; i < 6; i++) out[i] = ctx->tms[i];
   return SC_IVR_OK;
 }

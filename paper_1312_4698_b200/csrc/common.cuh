@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/sc_ivr.h"
 
 #define SCI_MAXF SC_IVR_MAX_F
@@ -49,8 +51,10 @@ struct sc_ivr_ctx {
   char err[512];
   int timing;
   double tms[6];
-  // timing events
-  cudaEvent_t ev[2];
+  // stage timing: (start, stop) event pairs recorded without synchronising, resolved by sc_ivr_last_timings
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> ev_slot;
+  size_t ev_used;
 };
 
 // kernel A launchers (propagate.cu)
