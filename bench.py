@@ -98,12 +98,12 @@ def cpu_oracle_sample(w, ntraj_sample: int, det_stride: int):
                 sample=f"first {ws.ntraj} trajectories of {w.name}, {w.nsteps} steps, {w.k} energies, det_stride={det_stride}: {dt:.1f} s"), dt
 
 
-def make_workload(config: int, rank: int, ntraj: int | None):
+def make_workload(config: int, rank: int, ntraj: int | None, nsteps: int | None = None, k: int | None = None):
     if rank == 0 and config != 5:
-        return inputs.make_config(config, ntraj=ntraj)
+        return inputs.make_config(config, ntraj=ntraj, nsteps=nsteps, k=k)
     # rank r > 0 (weak scaling): block r of config 5's 2^20-row draw on config 4's surface, same size as rank 0's
     n = ntraj or inputs._DEFAULTS[4 if config == 5 else config]["ntraj"]
-    full = inputs.make_config(5, ntraj=min((rank + 1) * n, 1 << 20))
+    full = inputs.make_config(5, ntraj=min((rank + 1) * n, 1 << 20), nsteps=nsteps, k=k)
     w = full.prefix(full.ntraj)
     w.p0q0 = np.ascontiguousarray(full.p0q0[:, full.ntraj - n:])
     return w
@@ -112,7 +112,7 @@ def make_workload(config: int, rank: int, ntraj: int | None):
 def run_reference(args, rank):
     if rank != 0:
         return
-    w = make_workload(args.config, 0, args.ntraj)
+    w = make_workload(args.config, 0, args.ntraj, args.nsteps, args.k)
     times = []
     for i in range(args.warmup + args.steps):
         cb, dt = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
@@ -138,6 +138,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--ntraj", type=int, default=None)
+    ap.add_argument("--nsteps", type=int, default=None)
+    ap.add_argument("--k", type=int, default=None)
     ap.add_argument("--det-stride", type=int, default=1)
     ap.add_argument("--ref-sample", type=int, default=1024)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -160,7 +162,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     B.lib()
 
-    w = make_workload(args.config, rank, args.ntraj)
+    w = make_workload(args.config, rank, args.ntraj, args.nsteps, args.k)
     ctx = B.ScIvr.from_workload(w, det_stride=args.det_stride)
     ctx.set_timing(True)
     d_pq = torch.from_numpy(w.p0q0).cuda()

@@ -71,6 +71,10 @@ typedef struct {
   int det_stride;  /* check det M every det_stride steps and at the last step; default 1 */
   double det_tol;  /* default 1e-6 */
   int integrator;  /* 0 = velocity-Verlet (default), 1 = 4-stage 4th-order symplectic */
+  double lu_growth_max; /* the two determinants are eliminated in a fixed pivot order while every multiplier of det K
+                           stays below lu_growth_max and every multiplier of det M below lu_growth_max^2; a step that
+                           exceeds them is repeated with pivoting.  0 = default 1e4;
+                           < 0 = always use the pivoted eliminations (testing) */
 } sc_ivr_options;
 
 /*

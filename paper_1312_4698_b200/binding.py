@@ -26,7 +26,8 @@ EXPORTS = [
 
 
 class sc_ivr_options(C.Structure):
-    _fields_ = [("det_stride", C.c_int), ("det_tol", C.c_double), ("integrator", C.c_int)]
+    _fields_ = [("det_stride", C.c_int), ("det_tol", C.c_double), ("integrator", C.c_int),
+                ("lu_growth_max", C.c_double)]
 
 
 class ScIvrError(RuntimeError):
@@ -121,11 +122,12 @@ def fp64_probe(mode=0, iters=20000):
 class ScIvr:
     """One context = one PES + (gamma, dt, nsteps, options).  Methods mirror the C entry points."""
 
-    def __init__(self, F, pes_kind, pes_coeffs, gamma, dt, nsteps, det_stride=1, det_tol=1e-6, integrator=0):
+    def __init__(self, F, pes_kind, pes_coeffs, gamma, dt, nsteps, det_stride=1, det_tol=1e-6, integrator=0,
+                 lu_growth_max=0.0):
         self._h = _vp(None)
         L = lib()
         co, ga = _host(pes_coeffs), _host(gamma)
-        opt = sc_ivr_options(int(det_stride), float(det_tol), int(integrator))
+        opt = sc_ivr_options(int(det_stride), float(det_tol), int(integrator), float(lu_growth_max))
         rc = L.sc_ivr_create(C.byref(self._h), int(F), int(pes_kind), _hp(co), co.size, _hp(ga), float(dt), int(nsteps),
                              C.byref(opt))
         if rc:

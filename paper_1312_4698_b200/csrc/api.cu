@@ -100,6 +100,18 @@ void fill_prop_params(const sc_ivr_ctx *ctx, PropParams &P, const double *chi) {
   P.coef = ctx->d_coef;
   P.det_tol = ctx->det_tol;
   P.det_stride = ctx->det_stride;
+  // thresholds of the static-order eliminations as IEEE high words (the kernel compares exponents + top mantissa bits)
+  auto hi_word = [](double x) {
+    unsigned long long u;
+    memcpy(&u, &x, sizeof(u));
+    return (unsigned)(u >> 32);
+  };
+  if (ctx->lu_growth_max < 0.0) {
+    P.grow_k_max = P.grow_m_max = 0u;
+  } else {
+    P.grow_k_max = hi_word(ctx->lu_growth_max);
+    P.grow_m_max = hi_word(ctx->lu_growth_max * ctx->lu_growth_max);
+  }
 }
 
 struct StageTimer {
@@ -159,6 +171,9 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
   int integrator = opt ? opt->integrator : 0;
   int det_stride = opt ? opt->det_stride : 1;
   double det_tol = opt ? opt->det_tol : 1e-6;
+  double lu_growth_max = opt ? opt->lu_growth_max : 0.0;
+  if (lu_growth_max == 0.0) lu_growth_max = 1e4;
+  if (!(lu_growth_max < 1e100)) return fail(ctx, SC_IVR_EINVAL, "bad lu_growth_max");
   if (det_stride == 0) det_stride = 1;
   if (det_tol == 0.0) det_tol = 1e-6;
   if (det_stride < 1 || !(det_tol > 0.0)) return fail(ctx, SC_IVR_EINVAL, "bad det_stride/det_tol");
@@ -178,6 +193,7 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
   ctx->dt = dt;
   ctx->det_stride = det_stride;
   ctx->det_tol = det_tol;
+  ctx->lu_growth_max = lu_growth_max;
   ctx->integrator = integrator;
   for (int a = 0; a < F; a++) {
     ctx->gamma[a] = gamma[a];

@@ -23,6 +23,7 @@ struct PropParams {
   int nsteps;
   int det_stride;
   double det_tol;
+  unsigned grow_k_max, grow_m_max;  // static-order LU: largest tolerated multiplier, as the high word of the double
   int nstages;
   double kick[SCI_MAX_STAGES];   // b_i * dt
   double drift[SCI_MAX_STAGES];  // a_i * dt
@@ -40,7 +41,7 @@ struct PropParams {
 
 struct sc_ivr_ctx {
   int F, kind, nsteps, det_stride, integrator;
-  double dt, det_tol;
+  double dt, det_tol, lu_growth_max;
   double gamma[SCI_MAXF], mass[SCI_MAXF];
   int nstages;
   double sa[SCI_MAX_STAGES], sb[SCI_MAX_STAGES];

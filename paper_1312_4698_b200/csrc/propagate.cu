@@ -38,7 +38,9 @@ struct Geo {
   static constexpr int FP = (F + 1) & ~1;  // F padded to even (16-byte alignment of the slots)
   static constexpr int NH = F * ND;
   static constexpr int NHP = (NH + 1) & ~1;
-  static constexpr int WS = FP + NHP + 2 * F;  // doubles of scratch per group: qs, Hs, red
+  static constexpr int KB = 2 * F;             // doubles per Herman-Kluk broadcast buffer (F double2)
+  static constexpr int MB = 2 * F + 2;         // doubles per monodromy broadcast buffer (reciprocal + 2F-1 rows, even)
+  static constexpr int WS = FP + NHP + 2 * F + 2 * KB + 2 * MB;  // doubles of scratch per group: qs, Hs, red, kb[2], mb[2]
   // packed coefficient block
   static constexpr int C3 = 0;                  // [ND][F][F]  (d, k, a) = Phi~[a][(a+d)%F][k]
   static constexpr int C4U = C3 + ND * F * F;   // [F][F]      (j, a) = P~[a][j]
@@ -254,6 +256,137 @@ __device__ __noinline__ double det_columns_real2(const double *C, int gbase, int
   return (par & 1u) ? -det : det;
 }
 
+// ---- a5 + a7, rare path: both determinants with pivoting, from the state AFTER the opening kick -------------------
+// st = (dP1, dQ1, dP2, dQ2) of the calling lane with the kick of weight bdt0 already applied; it is undone here with
+// H dQ recomputed from the group's Hessian slot (still the one of the current q).
+template <int F, int KIND>
+__device__ __noinline__ void pivoted_dets(const double *st, const double *Hs, double bdt0, int gbase, int a, unsigned gmask,
+                                          bool with_m, double &Dre, double &Dim, double &dM) {
+  double dP1[F], dQ1[F], dP2[F], dQ2[F], HM1[F], HM2[F];
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    dP1[i] = st[i];
+    dQ1[i] = st[F + i];
+    dP2[i] = st[2 * F + i];
+    dQ2[i] = st[3 * F + i];
+  }
+  hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
+  double buf[4 * F];
+  double Are[F], Aim[F];
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    const double p1 = fma(bdt0, HM1[i], dP1[i]), p2 = fma(bdt0, HM2[i], dP2[i]);
+    buf[i] = p1;
+    buf[F + i] = dQ1[i];
+    buf[2 * F + i] = p2;
+    buf[3 * F + i] = dQ2[i];
+    Are[i] = dQ2[i] + p1;
+    Aim[i] = p2 - dQ1[i];
+  }
+  det_columns_complex<F>(Are, Aim, gbase, a, gmask, Dre, Dim);
+  dM = with_m ? det_columns_real2<F>(buf, gbase, a, gmask) : 1.0;
+}
+
+// ---- a5 + a7, common path: both determinants by LU in a STATIC pivot order ---------------------------------------
+// Lane a owns column a of the F x F complex matrix 2K (Are, Aim) and columns a (C1) and F+a (C2) of the 2F x 2F
+// monodromy matrix, rows in (P, Q) order.  Step k eliminates row k with the diagonal pivot: the owner of column k
+// publishes (1/pivot, rest of its column) in a per-group shared-memory buffer (two buffers alternate, one
+// __syncwarp per step), every lane scales its row-k element by the reciprocal and updates its column(s).  The two
+// eliminations are independent and interleaved step by step so that each hides the other's latency.
+// No pivot search: the order is fixed, so there is no data-dependent control flow or register selection.  Its
+// numerical safety is monitored instead: grow = largest magnitude (IEEE high word) of any multiplier of a live
+// column.  A caller that sees grow above its bound repeats the step with the pivoted routines above (rare:
+// DESIGN.md "Static-order LU").  Results: on lane F-1, (Dre, Dim) = det(2K) * |R|^2 (a positive multiple of
+// det 2K: only its phase is used downstream, Eq. 10) and detM = det M.
+template <int F, bool WITH_M>
+__device__ __forceinline__ void lu_static(double (&Are)[F], double (&Aim)[F], double (&C1)[2 * F], double (&C2)[2 * F],
+                                          double2 *kb, double *mb, int a, unsigned amask, double &Dre, double &Dim,
+                                          double &detM, unsigned &growK, unsigned &growM) {
+  using X = Geo<F>;
+  constexpr int N = 2 * F;
+  constexpr int NSTEP = WITH_M ? N - 1 : F - 1;
+  double Rr = 1.0, Ri = 0.0, Rm = 1.0;
+  unsigned gk = 0u, gm = 0u;
+#pragma unroll
+  for (int k = 0; k < NSTEP; k++) {
+    const bool doK = k < F - 1;
+    if (doK) {
+      double2 *b = kb + (k & 1) * F;
+      const double rn = fast_rcp(fma(Are[k], Are[k], Aim[k] * Aim[k]));
+      if (a == k) {
+        b[0] = make_double2(Are[k] * rn, -Aim[k] * rn);
+#pragma unroll
+        for (int i = k + 1; i < F; i++) b[i - k] = make_double2(Are[i], Aim[i]);
+      }
+    }
+    if (WITH_M) {
+      double2 *b = reinterpret_cast<double2 *>(mb + (k & 1) * X::MB);
+      const bool own = (k < F) ? (a == k) : (a == k - F);
+      double(&C)[N] = (k < F) ? C1 : C2;
+      const double r = fast_rcp(C[k]);
+      if (own) {
+#pragma unroll
+        for (int t = 0; 2 * t < N - k; t++) {
+          const double x = (t == 0) ? r : C[k + 2 * t];
+          const double y = (k + 2 * t + 1 < N) ? C[k + 2 * t + 1] : 0.0;
+          b[t] = make_double2(x, y);
+        }
+      }
+    }
+    if (F > 1) __syncwarp(amask);
+    if (doK) {
+      const double2 *b = kb + (k & 1) * F;
+      const double2 r = b[0];
+      const double mr = Are[k] * r.x - Aim[k] * r.y;
+      const double mi = fma(Are[k], r.y, Aim[k] * r.x);
+      if (a > k) gk = max(gk, max((unsigned)__double2hiint(mr) & 0x7fffffffu, (unsigned)__double2hiint(mi) & 0x7fffffffu));
+      const double t = Rr * r.x - Ri * r.y;
+      Ri = fma(Rr, r.y, Ri * r.x);
+      Rr = t;
+#pragma unroll
+      for (int i = k + 1; i < F; i++) {
+        const double2 pv = b[i - k];
+        Are[i] = fma(-mr, pv.x, fma(mi, pv.y, Are[i]));
+        Aim[i] = fma(-mr, pv.y, fma(-mi, pv.x, Aim[i]));
+      }
+    }
+    if (WITH_M) {
+      const double2 *b = reinterpret_cast<const double2 *>(mb + (k & 1) * X::MB);
+      double2 pv = b[0];
+      const double r = pv.x;
+      Rm *= r;
+      const double m2 = C2[k] * r;
+      if (k < F || a > k - F) gm = max(gm, (unsigned)__double2hiint(m2) & 0x7fffffffu);
+      if (k < F) {
+        const double m1 = C1[k] * r;
+        if (a > k) gm = max(gm, (unsigned)__double2hiint(m1) & 0x7fffffffu);
+#pragma unroll
+        for (int i = k + 1; i < N; i++) {
+          const int e = i - k;
+          if ((e & 1) == 0) pv = b[e >> 1];
+          const double x = (e & 1) ? pv.y : pv.x;
+          C1[i] = fma(-m1, x, C1[i]);
+          C2[i] = fma(-m2, x, C2[i]);
+        }
+      } else {
+#pragma unroll
+        for (int i = k + 1; i < N; i++) {
+          const int e = i - k;
+          if ((e & 1) == 0) pv = b[e >> 1];
+          const double x = (e & 1) ? pv.y : pv.x;
+          C2[i] = fma(-m2, x, C2[i]);
+        }
+      }
+    }
+  }
+  // det 2K = p_{F-1} / R  ~  p_{F-1} conj(R);   det M = p_{2F-1} / R_m
+  Dre = fma(Are[F - 1], Rr, Aim[F - 1] * Ri);
+  Dim = fma(Aim[F - 1], Rr, -Are[F - 1] * Ri);
+  detM = WITH_M ? C2[N - 1] * fast_rcp(Rm) : 1.0;
+  growK = gk;
+  growM = gm;
+}
+
 template <int F, int KIND>
 __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ PropParams P) {
   using X = Geo<F>;
@@ -302,32 +435,75 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
   __syncwarp(X::AMASK);
   hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
 
+  double2 *kb = reinterpret_cast<double2 *>(ws + X::FP + X::NHP + 2 * F);
+  double *mb = ws + X::FP + X::NHP + 2 * F + 2 * X::KB;
+
   bool good = true;
   bool dirty = false;
   int det_count = 0;  // steps until the next check
   const int nsteps = P.nsteps;
 #pragma unroll 1
   for (int c = 0;; c++) {
-    // a5 (Eq. 5, R2): column a of 2K in reduced coordinates, then its determinant
-    double Dre, Dim;
-    {
-      double Are[F], Aim[F];
-#pragma unroll
-      for (int i = 0; i < F; i++) {
-        Are[i] = dQ2[i] + dP1[i];
-        Aim[i] = dP2[i] - dQ1[i];
-      }
-      det_columns_complex<F>(Are, Aim, gbase, a, gmask, Dre, Dim);
-    }
-    // a6 (Eq. 3): per-mode share of ln<chi|pq>; a8 input record
+    const bool last = (c == nsteps);
+    const bool check = (det_count == 0) || last;  // warp-uniform
+    // a6 (Eq. 3): per-mode share of ln<chi|pq> and of the phase S + arg<chi|pq>, at the integer time c
+    double oa = 0.0, ob = 0.0;
     if (P.raw != nullptr) {
       const double dq = Qeq_a - Q, dp = Peq_a - Pm;
-      const double oa = -0.25 * fma(dq, dq, dp * dp);
-      const double ob = 0.5 * (Peq_a + Pm) * dq;
+      oa = -0.25 * fma(dq, dq, dp * dp);
+      ob = fma(0.5 * (Peq_a + Pm), dq, Sa);
+      if (F > 1) red[a] = make_double2(oa, ob);
+    }
+    // working copies for the two eliminations: column a of 2K (a5; Eq. 5, R2) and columns a, F+a of M (a7)
+    double Are[F], Aim[F], C1[2 * F], C2[2 * F];
+#pragma unroll
+    for (int i = 0; i < F; i++) {
+      Are[i] = dQ2[i] + dP1[i];
+      Aim[i] = dP2[i] - dQ1[i];
+      C1[i] = dP1[i];
+      C1[F + i] = dQ1[i];
+      C2[i] = dP2[i];
+      C2[F + i] = dQ2[i];
+    }
+    // opening kick of the next step (stage 0), applied now so that H dQ is dead during the eliminations
+    const double bdt0 = last ? 0.0 : P.kick[0];
+    Sa = fma(-bdt0, Va, Sa);
+    Pm = fma(-bdt0, gq, Pm);
+#pragma unroll
+    for (int i = 0; i < F; i++) {
+      dP1[i] = fma(-bdt0, HM1[i], dP1[i]);
+      dP2[i] = fma(-bdt0, HM2[i], dP2[i]);
+    }
+    double Dre, Dim, dM;
+    unsigned growK, growM;
+    if (check) lu_static<F, true>(Are, Aim, C1, C2, kb, mb, a, X::AMASK, Dre, Dim, dM, growK, growM);
+    else lu_static<F, false>(Are, Aim, C1, C2, kb, mb, a, X::AMASK, Dre, Dim, dM, growK, growM);
+    {
+      // static order not safe for this matrix (or forced by the caller): repeat with the pivoted eliminations
+      const bool risky = (growK >= P.grow_k_max) || (check && growM >= P.grow_m_max);
+      const unsigned rb = __ballot_sync(X::AMASK, risky);
+      if (rb != 0u) {
+        double buf[4 * F];
+#pragma unroll
+        for (int i = 0; i < F; i++) {
+          buf[i] = dP1[i];
+          buf[F + i] = dQ1[i];
+          buf[2 * F + i] = dP2[i];
+          buf[3 * F + i] = dQ2[i];
+        }
+        double fDre, fDim, fdM;
+        pivoted_dets<F, KIND>(buf, Hs, bdt0, gbase, a, gmask, check, fDre, fDim, fdM);
+        if ((rb & gmask) != 0u) {
+          Dre = fDre;
+          Dim = fDim;
+          dM = fdM;
+        }
+      }
+    }
+    // a8 input record, written by the lane that holds the last pivots
+    if (P.raw != nullptr) {
       if (F > 1) {
-        red[a] = make_double2(oa, Sa + ob);
-        __syncwarp(X::AMASK);
-        if (a == 0) {
+        if (a == F - 1) {
           double s0 = 0.0, s1 = 0.0;
 #pragma unroll
           for (int i = 0; i < F; i++) {
@@ -338,42 +514,36 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
           if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre, Dim);
         }
       } else {
-        if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(oa, Sa + ob, Dre, Dim);
+        if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(oa, ob, Dre, Dim);
       }
     }
     // a7: |det M - 1| <= tol and finite, every det_stride steps and at the end
-    if (det_count == 0 || c == nsteps) {
-      double buf[4 * F];
-#pragma unroll
-      for (int i = 0; i < F; i++) {
-        buf[i] = dP1[i];
-        buf[F + i] = dQ1[i];
-        buf[2 * F + i] = dP2[i];
-        buf[3 * F + i] = dQ2[i];
-      }
-      const double dM = det_columns_real2<F>(buf, gbase, a, gmask);
-      const bool ok = (fabs(dM - 1.0) <= P.det_tol) && isfinite(Sa) && isfinite(Pm) && isfinite(Q);
-      good = good && ok;
+    if (check) {
+      const bool okd = (a == F - 1) ? (fabs(dM - 1.0) <= P.det_tol) : true;
+      good = good && okd && isfinite(Sa) && isfinite(Pm) && isfinite(Q);
       det_count = P.det_stride;
     }
     det_count--;
-    if (c == nsteps) break;
-    // a2-a4 (R10, R11): stages "kick b_i then drift a_i"; the PES is re-evaluated only after q moved
+    if (last) break;
+    // a2-a4 (R10, R11): stages "kick b_s then drift a_s"; stage 0's kick is already in; the PES is re-evaluated
+    // only after q moved
 #pragma unroll 1
     for (int st = 0; st < P.nstages; st++) {
-      if (dirty) {
-        pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
-        __syncwarp(X::AMASK);
-        hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
-        dirty = false;
-      }
-      const double bdt = P.kick[st];
-      Sa = fma(-bdt, Va, Sa);
-      Pm = fma(-bdt, gq, Pm);
+      if (st > 0) {
+        if (dirty) {
+          pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
+          __syncwarp(X::AMASK);
+          hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
+          dirty = false;
+        }
+        const double bdt = P.kick[st];
+        Sa = fma(-bdt, Va, Sa);
+        Pm = fma(-bdt, gq, Pm);
 #pragma unroll
-      for (int i = 0; i < F; i++) {
-        dP1[i] = fma(-bdt, HM1[i], dP1[i]);
-        dP2[i] = fma(-bdt, HM2[i], dP2[i]);
+        for (int i = 0; i < F; i++) {
+          dP1[i] = fma(-bdt, HM1[i], dP1[i]);
+          dP2[i] = fma(-bdt, HM2[i], dP2[i]);
+        }
       }
       const double adt = P.drift[st];
       if (adt != 0.0) {
@@ -387,6 +557,12 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
         }
         dirty = true;
       }
+    }
+    if (dirty) {  // schemes whose last drift is non-zero: the next step's opening kick needs the PES at the new q
+      pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
+      __syncwarp(X::AMASK);
+      hessian_times_tangent<F, KIND>(Hs, dQ1, dQ2, HM1, HM2);
+      dirty = false;
     }
   }
 

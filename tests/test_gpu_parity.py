@@ -98,6 +98,24 @@ def test_propagate_fourth_order_and_stride(torch_cuda, B, oracle):
     assert np.array_equal(o["good"].cpu().numpy(), r["good"])
 
 
+@pytest.mark.parametrize("growth", [-1.0, 1.5, 30.0], ids=["always_pivoted", "mixed_tight", "mixed_loose"])
+@pytest.mark.parametrize("cfg,ntraj", [(2, 203), (3, 77), (4, 100)])
+def test_propagate_static_and_pivoted_eliminations_agree_with_oracle(torch_cuda, B, oracle, cfg, ntraj, growth):
+    """a5, a7: the determinants come from a fixed-order elimination that falls back, per trajectory and step, to the
+    pivoted one when a multiplier grows beyond lu_growth_max.  Forcing the fallback always (-1) or often (a tight
+    bound, so that trajectories sharing a warp take different paths) must give the same z, theta and flags."""
+    torch = torch_cuda
+    w = inputs.make_config(cfg, ntraj=ntraj, nsteps=600, k=8)
+    ctx = B.ScIvr.from_workload(w, lu_growth_max=growth)
+    o = ctx.propagate(_dev(torch, w.p0q0), w.nsteps, chi=w.chi, want_z=True)
+    r = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, w.chi, want_z=True)
+    assert _relnorm(o["pq"].cpu().numpy(), r["pq"]) < TOL_STATE
+    assert _relnorm(o["S"].cpu().numpy(), r["S"]) < TOL_STATE
+    assert np.max(np.abs(o["theta"].cpu().numpy() - r["theta"])) < 1e-8
+    assert np.array_equal(o["good"].cpu().numpy(), r["good"])
+    assert np.max(np.abs(o["z"].cpu().numpy().T - r["z"])) < 1e-9
+
+
 def test_propagate_zero_steps(torch_cuda, B):
     """P0: M = I, S = 0, theta = 0, z_0 = <chi|p0 q0>; started at chi, z_0 = 1."""
     torch = torch_cuda
