@@ -1,7 +1,8 @@
 // Kernel A: fused PES (a1) + symplectic step (a2) + monodromy (a3) + action (a4) + Herman-Kluk
 // determinant (a5) + coherent-state overlap exponent (a6) + det M quality flag (a7).
 //
-// Mapping: F lanes per trajectory, G = floor(32/F) trajectories per warp.
+// Mapping: F lanes per trajectory, G = floor(32/F) trajectories per warp, lane = a * G + g
+// (a = mode / column index, g = trajectory of the warp).
 // Lane a of a group owns (P_a, Q_a), its share S_a of the action and the two tangent vectors
 // d(P,Q)/dP0_a and d(P,Q)/dQ0_a (columns a and F+a of the monodromy matrix, 2F doubles each), all in
 // registers.  The tangent map of a kick needs the full Hessian, so the lanes of a group compute
@@ -41,12 +42,15 @@ struct Geo {
   static constexpr int KB = 2 * F;             // doubles per Herman-Kluk broadcast buffer (F double2)
   static constexpr int MB = 2 * F + 2;         // doubles per monodromy broadcast buffer (reciprocal + 2F-1 rows, even)
   static constexpr int WS = FP + NHP + 2 * F + 2 * KB + 2 * MB;  // doubles of scratch per group: qs, Hs, red, kb[2], mb[2]
-  // packed coefficient block
-  static constexpr int C3 = 0;                  // [ND][F][F]  (d, k, a) = Phi~[a][(a+d)%F][k]
-  static constexpr int C4U = C3 + ND * F * F;   // [F][F]      (j, a) = P~[a][j]
-  static constexpr int C4D = C4U + F * F;       // [ND][F]     (d, a) = P~[a][(a+d)%F]
-  static constexpr int W2 = C4D + ND * F;       // [F]         omega_a^2 / gamma_a
-  static constexpr int NCOEF_QFF = W2 + F;
+  // packed coefficient block (QFF): lane a reads its own list of LA coefficients two at a time, pair t of lane a at
+  // double2 index t * F + a (adjacent lanes read adjacent 16-byte words).  Positions within the list:
+  static constexpr int L_C3 = 0;                // [ND][F]  (d, k) = Phi~[a][(a+d)%F][k]
+  static constexpr int L_C4U = L_C3 + ND * F;   // [F]      j      = P~[a][j]
+  static constexpr int L_C4D = L_C4U + F;       // [ND]     d      = P~[a][(a+d)%F]
+  static constexpr int L_W2 = L_C4D + ND;       //                   omega_a^2 / gamma_a
+  static constexpr int LA = L_W2 + 1;
+  static constexpr int LAP = (LA + 1) & ~1;
+  static constexpr int NCOEF_QFF = LAP * F;
   static constexpr int NCOEF_MORSE = 3 * F;     // D[F], a~[F], Qe[F]
   static constexpr int NCOEF = NCOEF_QFF > NCOEF_MORSE ? NCOEF_QFF : NCOEF_MORSE;
   static constexpr int NCOEFP = (NCOEF + 1) & ~1;
@@ -78,31 +82,41 @@ __device__ __forceinline__ void pes_group(const double *__restrict__ cs, double 
     qd[0] = Q;
 #pragma unroll
     for (int d = 1; d < X::ND; d++) qd[d] = qs[fwd[d]];
+    double cf[X::LAP];
+    {
+      const double2 *c2 = reinterpret_cast<const double2 *>(cs);
+#pragma unroll
+      for (int t = 0; t < X::LAP / 2; t++) {
+        const double2 v = c2[t * F + a];
+        cf[2 * t] = v.x;
+        cf[2 * t + 1] = v.y;
+      }
+    }
     double u = 0.0;
 #pragma unroll
-    for (int j = 0; j < F; j++) u = fma(cs[X::C4U + j * F + a], q[j] * q[j], u);
+    for (int j = 0; j < F; j++) u = fma(cf[X::L_C4U + j], q[j] * q[j], u);
     double h3[X::ND];
 #pragma unroll
     for (int d = 0; d < X::ND; d++) {
       double s = 0.0;
 #pragma unroll
-      for (int k = 0; k < F; k++) s = fma(cs[X::C3 + (d * F + k) * F + a], q[k], s);
+      for (int k = 0; k < F; k++) s = fma(cf[X::L_C3 + d * F + k], q[k], s);
       h3[d] = s;
     }
     double s3 = 0.0;
 #pragma unroll
     for (int d = 0; d < X::ND; d++) s3 = fma(h3[d], qd[d], s3);
 #pragma unroll
-    for (int d = 1; d <= X::NR; d++) s3 += __shfl_sync(X::AMASK, h3[d] * Q, gbase + bwd[d]);
-    const double w2 = cs[X::W2 + a];
-    const double paa = cs[X::C4D + a];
+    for (int d = 1; d <= X::NR; d++) s3 += __shfl_sync(X::AMASK, h3[d] * Q, bwd[d] * X::G + gbase);
+    const double w2 = cf[X::L_W2];
+    const double paa = cf[X::L_C4D];
     const double g3 = 0.5 * s3;
     const double g4 = Q * (0.5 * u - (1.0 / 3.0) * paa * Q * Q);
     g = fma(w2, Q, g3 + g4);
     Va = Q * (0.5 * w2 * Q + (1.0 / 3.0) * g3 + 0.25 * g4);
     Hent[0] = w2 + h3[0] + 0.5 * u;
 #pragma unroll
-    for (int d = 1; d < X::ND; d++) Hent[d] = fma(cs[X::C4D + d * F + a] * Q, qd[d], h3[d]);
+    for (int d = 1; d < X::ND; d++) Hent[d] = fma(cf[X::L_C4D + d] * Q, qd[d], h3[d]);
 #pragma unroll
     for (int d = 0; d < X::ND; d++) Hs[d * F + a] = Hent[d];
   } else {
@@ -168,7 +182,7 @@ __device__ __forceinline__ void det_columns_complex(double (&Are)[F], double (&A
     const unsigned key = used ? 0u : ((((unsigned)__double2hiint(mag)) & 0xFFFFFFE0u) | (unsigned)a) + 32u;
     const unsigned best = __reduce_max_sync(gmask, key);
     const int srcg = (int)((best - 32u) & 31u);
-    const int src = gbase + srcg;
+    const int src = srcg * X::G + gbase;
     par ^= __popc(umask & ((1u << srcg) - 1u));
     umask &= ~(1u << srcg);
     double pr[F], pi[F];
@@ -230,7 +244,7 @@ __device__ __noinline__ double det_columns_real2(const double *C, int gbase, int
     const int col = (int)((best - 32u) & 31u);
     const bool ssel = col >= F;
     const int srcg = ssel ? col - F : col;
-    const int src = gbase + srcg;
+    const int src = srcg * X::G + gbase;
     par ^= __popc(umask & ((1u << col) - 1u));
     umask &= ~(1u << col);
     double pv[N];
@@ -399,8 +413,12 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane >= X::ACT) return;
-  const int g = lane / F, a = lane - g * F, gbase = g * F;
-  const unsigned gmask = ((F == 32 ? 0u : (1u << F)) - 1u) << gbase;
+  // lane = a * G + g: the lanes that own the same column of the warp's G trajectories are adjacent, so that the
+  // owner's shared-memory stores of an elimination step fall into one quarter-warp (one wavefront instead of G)
+  const int a = lane / X::G, g = lane - a * X::G, gbase = g;
+  unsigned gmask = 0u;
+#pragma unroll
+  for (int i = 0; i < F; i++) gmask |= 1u << (i * X::G + g);
   double *ws = smem + X::NCOEFP + (warp * X::G + g) * X::WS;
   double *qs = ws, *Hs = ws + X::FP;
   double2 *red = reinterpret_cast<double2 *>(ws + X::FP + X::NHP);
@@ -573,7 +591,7 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
   if (F > 1) {
     Stot = 0.0;
 #pragma unroll
-    for (int i = 0; i < F; i++) Stot += __shfl_sync(X::AMASK, Sa, gbase + i);
+    for (int i = 0; i < F; i++) Stot += __shfl_sync(X::AMASK, Sa, i * X::G + gbase);
   }
   if (!valid) return;
   if (P.good != nullptr && a == 0) P.good[jj] = group_good ? 1 : 0;
@@ -612,7 +630,7 @@ __global__ void __launch_bounds__(kThreads) k_eval_pes(const double *__restrict_
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane >= X::ACT) return;
-  const int g = lane / F, a = lane - g * F, gbase = g * F;
+  const int a = lane / X::G, g = lane - a * X::G, gbase = g;
   double *ws = smem + X::NCOEFP + (warp * X::G + g) * X::WS;
   double *qs = ws, *Hs = ws + X::FP;
   const long long jj = (long long)blockIdx.x * (kThreads / 32 * X::G) + warp * X::G + g;
@@ -630,7 +648,7 @@ __global__ void __launch_bounds__(kThreads) k_eval_pes(const double *__restrict_
   pes_group<F, KIND>(cs, qs, Hs, a, gbase, fwd, bwd, Q, gq, Va, Hent);
   double Vt = 0.0;
 #pragma unroll
-  for (int i = 0; i < F; i++) Vt += __shfl_sync(X::AMASK, Va, gbase + i);
+  for (int i = 0; i < F; i++) Vt += __shfl_sync(X::AMASK, Va, i * X::G + gbase);
   if (!valid) return;
   if (a == 0) V[jl] = Vt;
   gout[(long long)a * n + jl] = gq * sg_a;
@@ -730,8 +748,8 @@ size_t sci_pack_coeffs(int F, int kind, const double *c, const double *gamma, do
     }
     return n;
   }
-  const int C3 = 0, C4U = C3 + ND * F * F, C4D = C4U + F * F, W2 = C4D + ND * F;
-  const size_t n = (size_t)W2 + F;
+  const int L_C3 = 0, L_C4U = L_C3 + ND * F, L_C4D = L_C4U + F, L_W2 = L_C4D + ND, LA = L_W2 + 1, LAP = (LA + 1) & ~1;
+  const size_t n = (size_t)LAP * F;
   if (!out) return n;
   // unpack the symmetric tensors
   double *phi = new double[(size_t)F * F * F];
@@ -752,14 +770,17 @@ size_t sci_pack_coeffs(int F, int kind, const double *c, const double *gamma, do
       const double v = qua[m++] / (gamma[i] * gamma[j]);
       pq[i * F + j] = pq[j * F + i] = v;
     }
-  for (int d = 0; d < ND; d++)
-    for (int k = 0; k < F; k++)
-      for (int a = 0; a < F; a++) out[C3 + (d * F + k) * F + a] = phi[((size_t)a * F + (a + d) % F) * F + k];
-  for (int j = 0; j < F; j++)
-    for (int a = 0; a < F; a++) out[C4U + j * F + a] = pq[a * F + j];
-  for (int d = 0; d < ND; d++)
-    for (int a = 0; a < F; a++) out[C4D + d * F + a] = pq[a * F + (a + d) % F];
-  for (int a = 0; a < F; a++) out[W2 + a] = c[a] * c[a] / gamma[a];
+  double *list = new double[LAP];
+  for (int a = 0; a < F; a++) {
+    for (int i = 0; i < LAP; i++) list[i] = 0.0;
+    for (int d = 0; d < ND; d++)
+      for (int k = 0; k < F; k++) list[L_C3 + d * F + k] = phi[((size_t)a * F + (a + d) % F) * F + k];
+    for (int j = 0; j < F; j++) list[L_C4U + j] = pq[a * F + j];
+    for (int d = 0; d < ND; d++) list[L_C4D + d] = pq[a * F + (a + d) % F];
+    list[L_W2] = c[a] * c[a] / gamma[a];
+    for (int i = 0; i < LAP; i++) out[((size_t)(i / 2) * F + a) * 2 + (i & 1)] = list[i];
+  }
+  delete[] list;
   delete[] phi;
   delete[] pq;
   return n;
