@@ -75,6 +75,9 @@ typedef struct {
                            stays below lu_growth_max and every multiplier of det M below lu_growth_max^2; a step that
                            exceeds them is repeated with pivoting.  0 = default 1e4;
                            < 0 = always use the pivoted eliminations (testing) */
+  int fourier_mode;     /* 0 = automatic: an equally spaced energy grid with nsteps + k <= 8192 takes the
+                           chirp-z (FFT) evaluation of the sum of Eq. 11, anything else the direct sum; 1 = always the
+                           direct sum */
 } sc_ivr_options;
 
 /*
@@ -162,12 +165,22 @@ sc_ivr_status sc_ivr_fourier(sc_ivr_ctx *ctx, const double *z, long long n, cons
                              double *A_out, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
+ * Parity / debug entry for step a8 through the chirp-z kernels that sc_ivr_run uses on equally spaced grids:
+ * P_out[j][i] = | sum_c z[c][j] e^{i E_i c dt} |^2.   z DEVICE [nsteps+1][n][2] (time-major), E HOST [k] equally spaced,
+ * P_out DEVICE [n][k], workspace DEVICE sc_ivr_fourier_power_workspace_bytes(ctx, n, k).
+ * SC_IVR_EUNSUPPORTED when the grid is not equally spaced or nsteps + k > 8192.
+ */
+size_t sc_ivr_fourier_power_workspace_bytes(const sc_ivr_ctx *ctx, long long n, int k);
+sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *z, long long n, const double *E, int k, double *P_out,
+                                   void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
  * Measurement helpers (no method arithmetic).
  * sc_ivr_fp64_probe: runs a register-only DFMA loop (mode 0) or an mma.sync m8n8k4 f64 loop (mode 1)
  * on every SM and returns the achieved FLOP/s (2 flop per FMA) in *flops_out.  Synchronous.
  * sc_ivr_last_timings: device times in ms (CUDA events on the run stream) of the stages of the most
- * recent sc_ivr_run on ctx, summed over batches: [0] propagate kernel, [1] z assembly, [2] twiddle table,
- * [3] Fourier kernel, [4] reduction kernels; [5] number of kernel launches.  Synchronises the stream's
+ * recent sc_ivr_run on ctx, summed over batches: [0] propagate kernel, [1] z assembly, [2] twiddle / chirp tables,
+ * [3] Fourier kernel (direct sum or chirp-z), [4] reduction kernels; [5] number of kernel launches.  Synchronises the stream's
  * last event.  Timing is recorded only after sc_ivr_set_timing(ctx, 1).
  */
 sc_ivr_status sc_ivr_fp64_probe(int mode, int iters, double *flops_out, double *ms_out);

@@ -21,13 +21,14 @@ EXPORTS = [
     "sc_ivr_create", "sc_ivr_destroy", "sc_ivr_last_error", "sc_ivr_workspace_bytes", "sc_ivr_min_batch",
     "sc_ivr_run", "sc_ivr_host_staging_bytes", "sc_ivr_run_host", "sc_ivr_propagate_workspace_bytes",
     "sc_ivr_propagate", "sc_ivr_eval_pes", "sc_ivr_fourier_workspace_bytes", "sc_ivr_fourier",
+    "sc_ivr_fourier_power_workspace_bytes", "sc_ivr_fourier_power",
     "sc_ivr_fp64_probe", "sc_ivr_set_timing", "sc_ivr_last_timings",
 ]
 
 
 class sc_ivr_options(C.Structure):
     _fields_ = [("det_stride", C.c_int), ("det_tol", C.c_double), ("integrator", C.c_int),
-                ("lu_growth_max", C.c_double)]
+                ("lu_growth_max", C.c_double), ("fourier_mode", C.c_int)]
 
 
 class ScIvrError(RuntimeError):
@@ -76,6 +77,10 @@ def lib():
     L.sc_ivr_eval_pes.argtypes = [_vp, _vp, C.c_longlong, _vp, _vp, _vp, _vp]
     L.sc_ivr_fourier_workspace_bytes.restype = C.c_size_t
     L.sc_ivr_fourier_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int]
+    L.sc_ivr_fourier_power_workspace_bytes.restype = C.c_size_t
+    L.sc_ivr_fourier_power_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int]
+    L.sc_ivr_fourier_power.restype = C.c_int
+    L.sc_ivr_fourier_power.argtypes = [_vp, _vp, C.c_longlong, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
     L.sc_ivr_fourier.restype = C.c_int
     L.sc_ivr_fourier.argtypes = [_vp, _vp, C.c_longlong, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
     L.sc_ivr_fp64_probe.restype = C.c_int
@@ -123,11 +128,11 @@ class ScIvr:
     """One context = one PES + (gamma, dt, nsteps, options).  Methods mirror the C entry points."""
 
     def __init__(self, F, pes_kind, pes_coeffs, gamma, dt, nsteps, det_stride=1, det_tol=1e-6, integrator=0,
-                 lu_growth_max=0.0):
+                 lu_growth_max=0.0, fourier_mode=0):
         self._h = _vp(None)
         L = lib()
         co, ga = _host(pes_coeffs), _host(gamma)
-        opt = sc_ivr_options(int(det_stride), float(det_tol), int(integrator), float(lu_growth_max))
+        opt = sc_ivr_options(int(det_stride), float(det_tol), int(integrator), float(lu_growth_max), int(fourier_mode))
         rc = L.sc_ivr_create(C.byref(self._h), int(F), int(pes_kind), _hp(co), co.size, _hp(ga), float(dt), int(nsteps),
                              C.byref(opt))
         if rc:
@@ -243,6 +248,17 @@ class ScIvr:
         H = torch.empty((F, F, n), dtype=torch.float64, device=dev)
         self._check(lib().sc_ivr_eval_pes(self._h, _dev(q), n, _dev(V), _dev(g), _dev(H), _stream()))
         return V, g, H
+
+    def fourier_power(self, z, E):
+        """sc_ivr_fourier_power (chirp-z kernels): z DEVICE complex [nsteps+1, n] -> |A|^2 DEVICE [n, k]."""
+        import torch
+        assert z.is_cuda and z.dtype == torch.complex128 and z.is_contiguous() and z.shape[0] == self.nsteps + 1
+        n, dev = z.shape[1], z.device
+        E = _host(E)
+        P = torch.empty((n, E.size), dtype=torch.float64, device=dev)
+        ws = _workspace(lib().sc_ivr_fourier_power_workspace_bytes(self._h, n, E.size), dev)
+        self._check(lib().sc_ivr_fourier_power(self._h, _dev(z), n, _hp(E), E.size, _dev(P), _dev(ws), ws.numel(), _stream()))
+        return P
 
     def fourier(self, z, E):
         """sc_ivr_fourier: z DEVICE complex [nsteps+1, n] (time-major) -> A DEVICE complex [n, k]."""

@@ -46,7 +46,8 @@ struct Carve {
   long long nbp;        // nbatch rounded to the Fourier tile (z row stride)
   int rows, zrows, kp;  // nsteps+1, rows padded to KC, k padded to TI
   long long tiles_total;
-  size_t off_raw, off_z, off_W, off_partial, off_good, off_wg, off_E, off_ngood, total;
+  long long xstride;    // chirp path: row stride of x[j][c] (rows = nsteps+1 rounded up to 32)
+  size_t off_raw, off_z, off_W, off_partial, off_good, off_wg, off_E, off_ngood, off_pc, off_hrow, off_HpT, total;
 };
 
 Carve carve(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
@@ -58,15 +59,23 @@ Carve carve(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
   c.kp = (int)round_up_ll(k, SCI_TI);
   const long long nbatches = (ntraj + nbatch - 1) / nbatch;
   c.tiles_total = nbatches * (c.nbp / SCI_TJ);
+  if (c.tiles_total < nbatches * ctx->sm_count) c.tiles_total = nbatches * ctx->sm_count;  // chirp path: one partial per CTA
+  c.xstride = round_up_ll(c.rows, 32);
+  size_t zbytes = sizeof(double2) * (size_t)c.zrows * (size_t)c.nbp;                   // direct path: z[c][j]
+  const size_t xbytes = sizeof(double2) * (size_t)c.xstride * (size_t)nbatch;          // chirp path:  x[j][c]
+  if (xbytes > zbytes) zbytes = xbytes;
   size_t o = 0;
   c.off_raw = o; o = align_up(o + sizeof(double4) * (size_t)c.rows * (size_t)nbatch, 256);
-  c.off_z = o; o = align_up(o + sizeof(double2) * (size_t)c.zrows * (size_t)c.nbp, 256);
+  c.off_z = o; o = align_up(o + zbytes, 256);
   c.off_W = o; o = align_up(o + sizeof(double2) * (size_t)c.zrows * (size_t)c.kp, 256);
   c.off_partial = o; o = align_up(o + sizeof(double) * (size_t)c.tiles_total * (size_t)c.kp, 256);
   c.off_good = o; o = align_up(o + (size_t)ntraj, 256);
   c.off_wg = o; o = align_up(o + sizeof(double) * (size_t)ntraj, 256);
   c.off_E = o; o = align_up(o + sizeof(double) * (size_t)k, 256);
   c.off_ngood = o; o = align_up(o + 64, 256);
+  c.off_pc = o; o = align_up(o + sizeof(double2) * (size_t)c.rows, 256);
+  c.off_hrow = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L, 256);
+  c.off_HpT = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L, 256);
   c.total = o;
   return c;
 }
@@ -112,6 +121,27 @@ void fill_prop_params(const sc_ivr_ctx *ctx, PropParams &P, const double *chi) {
     P.grow_k_max = hi_word(ctx->lu_growth_max);
     P.grow_m_max = hi_word(ctx->lu_growth_max * ctx->lu_growth_max);
   }
+}
+
+// Equally spaced grid?  E_i = E_0 + i dE to within a few ulp of the largest |E|.
+bool uniform_grid(const double *E, int k, double *e0, double *de) {
+  *e0 = E[0];
+  *de = k > 1 ? (E[k - 1] - E[0]) / (double)(k - 1) : 0.0;
+  double emax = 0.0;
+  for (int i = 0; i < k; i++) {
+    if (!isfinite(E[i])) return false;
+    emax = fmax(emax, fabs(E[i]));
+  }
+  const double tol = 8.0 * 2.220446049250313e-16 * emax;
+  for (int i = 0; i < k; i++)
+    if (fabs(E[i] - (*e0 + (double)i * *de)) > tol) return false;
+  return true;
+}
+
+bool chirp_applies(const sc_ivr_ctx *ctx, const double *E, int k, double *e0, double *de) {
+  if (ctx->fourier_mode == 1) return false;
+  if ((long long)ctx->nsteps + (long long)k > SCI_CHIRP_L) return false;
+  return uniform_grid(E, k, e0, de);
 }
 
 struct StageTimer {
@@ -178,6 +208,8 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
   if (det_tol == 0.0) det_tol = 1e-6;
   if (det_stride < 1 || !(det_tol > 0.0)) return fail(ctx, SC_IVR_EINVAL, "bad det_stride/det_tol");
   if (integrator != 0 && integrator != 1) return fail(ctx, SC_IVR_EUNSUPPORTED, "unknown integrator %d", integrator);
+  const int fourier_mode = opt ? opt->fourier_mode : 0;
+  if (fourier_mode != 0 && fourier_mode != 1) return fail(ctx, SC_IVR_EUNSUPPORTED, "unknown fourier_mode %d", fourier_mode);
 
   int ndev = 0;
   cudaError_t ce = cudaGetDeviceCount(&ndev);
@@ -195,6 +227,7 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
   ctx->det_tol = det_tol;
   ctx->lu_growth_max = lu_growth_max;
   ctx->integrator = integrator;
+  ctx->fourier_mode = fourier_mode;
   for (int a = 0; a < F; a++) {
     ctx->gamma[a] = gamma[a];
     ctx->mass[a] = (kind == SC_IVR_PES_QFF) ? 1.0 : pes_coeffs[4 * a + 3];
@@ -324,11 +357,23 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
   StageTimer tm(ctx, st);
   double launches = 0;
 
-  CU(cudaMemcpyAsync(E_dev, E, sizeof(double) * k, cudaMemcpyHostToDevice, st));
+  double2 *pc = (double2 *)(ws + cv.off_pc);
+  double2 *hrow = (double2 *)(ws + cv.off_hrow);
+  double2 *HpT = (double2 *)(ws + cv.off_HpT);
+  double e0 = 0.0, de = 0.0;
+  const bool chirp = chirp_applies(ctx, E, k, &e0, &de);
+  const int chirp_grid = ctx->sm_count;
   tm.begin();
-  CU(sci_launch_twiddle(E_dev, k, cv.kp, cv.zrows, ctx->dt, W, st));
+  if (chirp) {  // inner chirp, filter row, filter spectrum (one FFT)
+    CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, cv.rows, k, pc, hrow, st));
+    CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, cv.kp, nullptr, HpT, 1, st));
+    launches += 2;
+  } else {
+    CU(cudaMemcpyAsync(E_dev, E, sizeof(double) * k, cudaMemcpyHostToDevice, st));
+    CU(sci_launch_twiddle(E_dev, k, cv.kp, cv.zrows, ctx->dt, W, st));
+    launches += 1;
+  }
   tm.end(2);
-  launches += 1;
 
   PropParams P;
   fill_prop_params(ctx, P, chi);
@@ -349,15 +394,22 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
     CU(sci_launch_propagate(F, ctx->kind, P, st));
     tm.end(0);
     tm.begin();
-    CU(sci_launch_zassemble(raw, cv.nbatch, nb, ctx->nsteps, z, cv.nbp, zcols, cv.zrows, nullptr, st));
+    if (chirp) CU(sci_launch_zassemble_rows(raw, cv.nbatch, nb, ctx->nsteps, pc, z, cv.xstride, st));
+    else CU(sci_launch_zassemble(raw, cv.nbatch, nb, ctx->nsteps, z, cv.nbp, zcols, cv.zrows, nullptr, st));
     tm.end(1);
     tm.begin();
     CU(sci_launch_weights(weights ? weights + j0 : nullptr, good + j0, nb, wg + j0, st));
     tm.end(4);
     tm.begin();
-    CU(sci_launch_fourier(z, cv.nbp, zcols, cv.zrows, W, cv.kp, nb, wg + j0, partial + tile0 * cv.kp, nullptr, k, st));
+    if (chirp) {
+      const int grid = nb < chirp_grid ? (int)nb : chirp_grid;
+      CU(sci_launch_chirp_fft(0, z, cv.xstride, cv.rows, nb, HpT, wg + j0, k, cv.kp, partial + tile0 * cv.kp, nullptr, grid, st));
+      tile0 += grid;
+    } else {
+      CU(sci_launch_fourier(z, cv.nbp, zcols, cv.zrows, W, cv.kp, nb, wg + j0, partial + tile0 * cv.kp, nullptr, k, st));
+      tile0 += zcols / SCI_TJ;
+    }
     tm.end(3);
-    tile0 += zcols / SCI_TJ;
     launches += 4;
   }
   tm.begin();
@@ -475,6 +527,38 @@ sc_ivr_status sc_ivr_fourier(sc_ivr_ctx *ctx, const double *zin, long long n, co
   CU(cudaMemcpyAsync(E_dev, E, sizeof(double) * k, cudaMemcpyHostToDevice, st));
   CU(sci_launch_twiddle(E_dev, k, kp, zrows, ctx->dt, W, st));
   CU(sci_launch_fourier(z, ncp, ncp, zrows, W, kp, n, nullptr, nullptr, (double2 *)A_out, k, st));
+  return SC_IVR_OK;
+}
+
+size_t sc_ivr_fourier_power_workspace_bytes(const sc_ivr_ctx *ctx, long long n, int k) {
+  if (!ctx || n < 1 || k < 1) return 0;
+  const size_t rows = (size_t)ctx->nsteps + 1, xstride = (size_t)round_up_ll((long long)rows, 32);
+  return align_up(sizeof(double2) * xstride * (size_t)n, 256) + align_up(sizeof(double2) * rows, 256) +
+         2 * align_up(sizeof(double2) * SCI_CHIRP_L, 256);
+}
+
+sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *zin, long long n, const double *E, int k, double *P_out,
+                                   void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!zin || !E || !P_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (n < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "n and k must be >= 1");
+  if (workspace_bytes < sc_ivr_fourier_power_workspace_bytes(ctx, n, k)) return fail(ctx, SC_IVR_EINVAL, "workspace too small");
+  double e0 = 0.0, de = 0.0;
+  if ((long long)ctx->nsteps + (long long)k > SCI_CHIRP_L || !uniform_grid(E, k, &e0, &de))
+    return fail(ctx, SC_IVR_EUNSUPPORTED, "chirp-z needs an equally spaced grid and nsteps + k <= %d", SCI_CHIRP_L);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int rows = ctx->nsteps + 1;
+  const long long xstride = round_up_ll(rows, 32);
+  char *ws = (char *)workspace;
+  double2 *x = (double2 *)ws;
+  double2 *pc = (double2 *)(ws + align_up(sizeof(double2) * (size_t)xstride * (size_t)n, 256));
+  double2 *hrow = (double2 *)((char *)pc + align_up(sizeof(double2) * (size_t)rows, 256));
+  double2 *HpT = (double2 *)((char *)hrow + align_up(sizeof(double2) * SCI_CHIRP_L, 256));
+  CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, rows, k, pc, hrow, st));
+  CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, k, nullptr, HpT, 1, st));
+  CU(sci_launch_rows_from_z((const double2 *)zin, n, rows, pc, x, xstride, st));
+  const int grid = n < ctx->sm_count ? (int)n : ctx->sm_count;
+  CU(sci_launch_chirp_fft(2, x, xstride, rows, n, HpT, nullptr, k, k, P_out, nullptr, grid, st));
   return SC_IVR_OK;
 }
 

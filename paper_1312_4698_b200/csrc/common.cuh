@@ -40,7 +40,7 @@ struct PropParams {
 };
 
 struct sc_ivr_ctx {
-  int F, kind, nsteps, det_stride, integrator;
+  int F, kind, nsteps, det_stride, integrator, fourier_mode;
   double dt, det_tol, lu_growth_max;
   double gamma[SCI_MAXF], mass[SCI_MAXF];
   int nstages;
@@ -81,3 +81,14 @@ cudaError_t sci_launch_count_good(const unsigned char *good, long long n, long l
 cudaError_t sci_launch_final(const double *partial, long long ntiles, int kp, int k, const long long *ngood, double norm_no_ngood,
                              double *I_out, cudaStream_t st);
 cudaError_t sci_fp64_probe(int mode, int iters, double *flops, double *ms);
+
+// chirp-z Fourier stage for equally spaced energy grids (chirp.cu)
+#define SCI_CHIRP_L 8192  // circular convolution length: the fast path needs (nsteps + 1) + k - 1 <= SCI_CHIRP_L
+size_t sci_chirp_smem_bytes();
+cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, double2 *pc, double2 *hrow, cudaStream_t st);
+cudaError_t sci_launch_zassemble_rows(const double4 *raw, long long raw_stride, long long nb, int nsteps, const double2 *pc,
+                                      double2 *xrows, long long xstride, cudaStream_t st);
+cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const double2 *pc, double2 *xrows, long long xstride,
+                                   cudaStream_t st);
+cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, int n1, long long nrows, const double2 *HpT,
+                                 const double *wg, int k, int kp, double *out, double2 *spec_out, int grid, cudaStream_t st);

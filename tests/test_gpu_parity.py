@@ -148,6 +148,51 @@ def test_fourier_parity(torch_cuda, B, oracle):
     assert np.max(np.abs(A - Ao)) < 1e-11 * np.max(np.abs(Ao))
 
 
+@pytest.mark.parametrize("nsteps,n,k,emin,emax", [(333, 150, 70, 0.0, 20000.0), (4000, 37, 4000, 0.0, 20000.0),
+                                                 (4191, 5, 4000, 1500.0, 9000.0), (1, 3, 1, 700.0, 700.0),
+                                                 (2999, 9, 2000, -3000.0, 20000.0)])
+def test_fourier_chirp_z_parity(torch_cuda, B, oracle, nsteps, n, k, emin, emax):
+    """a8 on an equally spaced grid: |A_j(E_i)|^2 from the chirp-z (FFT) kernels vs the definition
+    (one cexp per term) in the oracle; sizes up to the limit nsteps + k = 8191 + 1, grids that do not start at 0."""
+    torch = torch_cuda
+    rng = np.random.default_rng(11)
+    w = inputs.make_config(1, ntraj=2, nsteps=nsteps, k=k)
+    E = inputs.energy_grid(k, emin, emax)
+    z = (rng.standard_normal((n, nsteps + 1)) + 1j * rng.standard_normal((n, nsteps + 1))) * 0.3
+    z[:, ::7] *= 3.0
+    ctx = B.ScIvr.from_workload(w)
+    P = ctx.fourier_power(_dev(torch, z.T.copy()), E).cpu().numpy()
+    Po = np.abs(oracle.fourier(z, w.dt, E, mode=0 if nsteps * k < 2_000_000 else 1)) ** 2
+    assert np.max(np.abs(P - Po)) < 1e-10 * np.max(Po)
+
+
+def test_fourier_chirp_z_refuses_what_it_cannot_do(torch_cuda, B):
+    torch = torch_cuda
+    w = inputs.make_config(1, ntraj=2, nsteps=100, k=16)
+    ctx = B.ScIvr.from_workload(w)
+    z = torch.zeros((101, 4), dtype=torch.complex128, device="cuda")
+    E = w.E.copy()
+    E[5] *= 1.0 + 1e-9  # not equally spaced
+    with pytest.raises(B.ScIvrError) as ei:
+        ctx.fourier_power(z, E)
+    assert ei.value.status == 4
+
+
+@pytest.mark.parametrize("mode", ["direct_forced", "direct_nonuniform_grid", "chirp"])
+def test_run_fourier_paths_agree_with_oracle(torch_cuda, B, oracle, mode):
+    """sc_ivr_run takes the chirp-z path on an equally spaced grid and the direct sum otherwise (or when forced);
+    both must match the oracle on the same inputs."""
+    torch = torch_cuda
+    w = inputs.make_config(3, ntraj=333, nsteps=700, k=300)
+    if mode == "direct_nonuniform_grid":
+        w.E = w.E + 1e-7 * np.sin(np.arange(w.k))  # breaks equal spacing far beyond rounding
+    ctx = B.ScIvr.from_workload(w, fourier_mode=1 if mode == "direct_forced" else 0)
+    I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
+    Io, ngo, rco = oracle.run_workload(w)
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I.cpu().numpy(), Io)
+
+
 def _run_both(torch, B, oracle, w, **kw):
     ctx = B.ScIvr.from_workload(w, **kw)
     I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
