@@ -36,11 +36,14 @@ UNIT = "trajectory-steps/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the bench configuration,
 # from the ncu --set full capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = {"propagate": None, "fourier": None}
+NCU_TRAFFIC_BYTES = {"propagate": 16974059640, "fourier": None}  # profiles/r01c_kernelA_full_config4.md
+CHIRP_L = 8192  # circular convolution length of the chirp-z Fourier stage (csrc/common.cuh SCI_CHIRP_L)
 
 
-def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False):
-    """Algorithmic flop per trajectory-step (SURVEY.md 8d table, 1 FMA = 2 flop)."""
+def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False, nsteps: int = 4000, chirp: bool = True):
+    """Algorithmic flop per trajectory-step (SURVEY.md 8d table, 1 FMA = 2 flop).  Fourier stage: the direct sum of
+    Eq. 11 is 8k per trajectory-step; on an equally spaced grid the library evaluates it as a chirp-z transform
+    (two FFTs of length 8192 per trajectory), whose own count 2 * 5 L log2 L / (nsteps + 1) is what is credited."""
     pes = 60 if morse else 2 * (F * F * (F + 1) // 2 + 2 * F * F + F * (F - 1) + 6 * F)
     step = 16 * F + 6
     mono = 2 * (2 * F ** 3 + 6 * F ** 2)
@@ -52,7 +55,8 @@ def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False):
     check = 2 * ((n - 1) * n * (2 * n - 1) // 6) + n * (n - 1) // 2 + 12 * n
     if det_every_step:
         a_total += check
-    return dict(propagate=a_total, fourier=8 * k)
+    fourier = 2 * 5 * CHIRP_L * math.log2(CHIRP_L) / (nsteps + 1) if chirp else 8 * k
+    return dict(propagate=a_total, fourier=fourier)
 
 
 class ClockSampler(threading.Thread):
@@ -222,7 +226,9 @@ def main():
     e2e_value = units / (e2e_ms * 1e-3)
 
     if rank == 0:
-        fm = flop_model(w.F, w.k, args.det_stride == 1, morse=(w.pes_kind != inputs.PES_QFF))
+        chirp = (w.nsteps + w.k <= CHIRP_L)  # inputs.energy_grid is equally spaced
+        fm = flop_model(w.F, w.k, args.det_stride == 1, morse=(w.pes_kind != inputs.PES_QFF), nsteps=w.nsteps, chirp=chirp)
+        kname = {"propagate": "k_propagate", "fourier": "k_chirp_fft" if chirp else "k_fourier"}
         dom = "fourier" if stage["fourier_ms"] >= stage["propagate_ms"] else "propagate"
         dom_ms = stage[dom + "_ms"]
         flops_per_launch = fm[dom] * w.ntraj * w.nsteps  # one launch per run when the workload is a single batch
@@ -248,11 +254,11 @@ def main():
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.p0q0.nbytes + w.E.nbytes),
                     "d2h_bytes_per_step": int(w.k * 8 + 8)},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": kname[dom], "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES[dom],
                          "peak_source": "148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); this run's FP64 probes alongside",
                          "flop_per_trajectory_step": fm[dom], "probe": probe,
-                         "other_kernel": {"kernel": "k_" + other, "achieved": other_tf, "frac": other_tf / FP64_PEAK_TFLOPS,
+                         "other_kernel": {"kernel": kname[other], "achieved": other_tf, "frac": other_tf / FP64_PEAK_TFLOPS,
                                           "flop_per_trajectory_step": fm[other]}},
             "stage_ms_last_step": stage,
             "cpu_baseline": cpu,
