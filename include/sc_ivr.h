@@ -75,9 +75,9 @@ typedef struct {
                            stays below lu_growth_max and every multiplier of det M below lu_growth_max^2; a step that
                            exceeds them is repeated with pivoting.  0 = default 1e4;
                            < 0 = always use the pivoted eliminations (testing) */
-  int fourier_mode;     /* 0 = automatic: an equally spaced energy grid with nsteps + k <= 8192 takes the
-                           chirp-z (FFT) evaluation of the sum of Eq. 11, anything else the direct sum; 1 = always the
-                           direct sum */
+  int fourier_mode;     /* 0 = automatic: an equally spaced energy grid with k <= 7169 and at most 16
+                           blocks of 8193 - k time samples takes the chirp-z (FFT) evaluation of the sum of Eq. 11,
+                           anything else the direct sum; 1 = always the direct sum */
 } sc_ivr_options;
 
 /*
@@ -168,7 +168,7 @@ sc_ivr_status sc_ivr_fourier(sc_ivr_ctx *ctx, const double *z, long long n, cons
  * Parity / debug entry for step a8 through the chirp-z kernels that sc_ivr_run uses on equally spaced grids:
  * P_out[j][i] = | sum_c z[c][j] e^{i E_i c dt} |^2.   z DEVICE [nsteps+1][n][2] (time-major), E HOST [k] equally spaced,
  * P_out DEVICE [n][k], workspace DEVICE sc_ivr_fourier_power_workspace_bytes(ctx, n, k).
- * SC_IVR_EUNSUPPORTED when the grid is not equally spaced or nsteps + k > 8192.
+ * SC_IVR_EUNSUPPORTED when the grid is not equally spaced, k > 7169 or the series needs more than 16 blocks.
  */
 size_t sc_ivr_fourier_power_workspace_bytes(const sc_ivr_ctx *ctx, long long n, int k);
 sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *z, long long n, const double *E, int k, double *P_out,

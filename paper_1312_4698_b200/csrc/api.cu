@@ -47,7 +47,7 @@ struct Carve {
   int rows, zrows, kp;  // nsteps+1, rows padded to KC, k padded to TI
   long long tiles_total;
   long long xstride;    // chirp path: row stride of x[j][c] (rows = nsteps+1 rounded up to 32)
-  size_t off_raw, off_z, off_W, off_partial, off_good, off_wg, off_E, off_ngood, off_pc, off_hrow, off_HpT, total;
+  size_t off_raw, off_z, off_W, off_partial, off_good, off_wg, off_E, off_ngood, off_pc, off_hrow, off_HpT, off_yscr, total;
 };
 
 Carve carve(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
@@ -74,8 +74,9 @@ Carve carve(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
   c.off_E = o; o = align_up(o + sizeof(double) * (size_t)k, 256);
   c.off_ngood = o; o = align_up(o + 64, 256);
   c.off_pc = o; o = align_up(o + sizeof(double2) * (size_t)c.rows, 256);
-  c.off_hrow = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L, 256);
-  c.off_HpT = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L, 256);
+  c.off_hrow = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256);
+  c.off_HpT = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256);
+  c.off_yscr = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L * (size_t)ctx->sm_count, 256);
   c.total = o;
   return c;
 }
@@ -138,9 +139,20 @@ bool uniform_grid(const double *E, int k, double *e0, double *de) {
   return true;
 }
 
-bool chirp_applies(const sc_ivr_ctx *ctx, const double *E, int k, double *e0, double *de) {
+// Chirp-z plan: blocks of bsz = L - k + 1 time samples.
+bool chirp_plan(int nsteps, int k, int *nblocks, int *bsz) {
+  const long long b = (long long)SCI_CHIRP_L - k + 1;
+  if (b < SCI_CHIRP_MIN_BLOCK) return false;
+  const long long nb = ((long long)nsteps + 1 + b - 1) / b;
+  if (nb > SCI_CHIRP_MAX_BLOCKS) return false;
+  *nblocks = (int)nb;
+  *bsz = (int)b;
+  return true;
+}
+
+bool chirp_applies(const sc_ivr_ctx *ctx, const double *E, int k, double *e0, double *de, int *nblocks, int *bsz) {
   if (ctx->fourier_mode == 1) return false;
-  if ((long long)ctx->nsteps + (long long)k > SCI_CHIRP_L) return false;
+  if (!chirp_plan(ctx->nsteps, k, nblocks, bsz)) return false;
   return uniform_grid(E, k, e0, de);
 }
 
@@ -360,14 +372,16 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
   double2 *pc = (double2 *)(ws + cv.off_pc);
   double2 *hrow = (double2 *)(ws + cv.off_hrow);
   double2 *HpT = (double2 *)(ws + cv.off_HpT);
+  double2 *yscr = (double2 *)(ws + cv.off_yscr);
   double e0 = 0.0, de = 0.0;
-  const bool chirp = chirp_applies(ctx, E, k, &e0, &de);
+  int cblocks = 1, cbsz = 0;
+  const bool chirp = chirp_applies(ctx, E, k, &e0, &de, &cblocks, &cbsz);
   const int chirp_grid = ctx->sm_count;
   tm.begin();
-  if (chirp) {  // inner chirp, filter row, filter spectrum (one FFT)
-    CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, cv.rows, k, pc, hrow, st));
-    CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, cv.kp, nullptr, HpT, 1, st));
-    launches += 2;
+  if (chirp) {  // inner chirp, filter rows, filter spectra (one FFT per block)
+    CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, cv.rows, k, cblocks, cbsz, pc, hrow, st));
+    CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, cv.kp, nullptr, HpT, cblocks, cbsz, nullptr, 1, st));
+    launches += 1 + cblocks;
   } else {
     CU(cudaMemcpyAsync(E_dev, E, sizeof(double) * k, cudaMemcpyHostToDevice, st));
     CU(sci_launch_twiddle(E_dev, k, cv.kp, cv.zrows, ctx->dt, W, st));
@@ -403,7 +417,8 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
     tm.begin();
     if (chirp) {
       const int grid = nb < chirp_grid ? (int)nb : chirp_grid;
-      CU(sci_launch_chirp_fft(0, z, cv.xstride, cv.rows, nb, HpT, wg + j0, k, cv.kp, partial + tile0 * cv.kp, nullptr, grid, st));
+      CU(sci_launch_chirp_fft(0, z, cv.xstride, cv.rows, nb, HpT, wg + j0, k, cv.kp, partial + tile0 * cv.kp, nullptr, cblocks, cbsz, yscr, grid,
+                              st));
       tile0 += grid;
     } else {
       CU(sci_launch_fourier(z, cv.nbp, zcols, cv.zrows, W, cv.kp, nb, wg + j0, partial + tile0 * cv.kp, nullptr, k, st));
@@ -534,7 +549,8 @@ size_t sc_ivr_fourier_power_workspace_bytes(const sc_ivr_ctx *ctx, long long n, 
   if (!ctx || n < 1 || k < 1) return 0;
   const size_t rows = (size_t)ctx->nsteps + 1, xstride = (size_t)round_up_ll((long long)rows, 32);
   return align_up(sizeof(double2) * xstride * (size_t)n, 256) + align_up(sizeof(double2) * rows, 256) +
-         2 * align_up(sizeof(double2) * SCI_CHIRP_L, 256);
+         2 * align_up(sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256) +
+         align_up(sizeof(double2) * SCI_CHIRP_L * (size_t)ctx->sm_count, 256);
 }
 
 sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *zin, long long n, const double *E, int k, double *P_out,
@@ -544,8 +560,10 @@ sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *zin, long long
   if (n < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "n and k must be >= 1");
   if (workspace_bytes < sc_ivr_fourier_power_workspace_bytes(ctx, n, k)) return fail(ctx, SC_IVR_EINVAL, "workspace too small");
   double e0 = 0.0, de = 0.0;
-  if ((long long)ctx->nsteps + (long long)k > SCI_CHIRP_L || !uniform_grid(E, k, &e0, &de))
-    return fail(ctx, SC_IVR_EUNSUPPORTED, "chirp-z needs an equally spaced grid and nsteps + k <= %d", SCI_CHIRP_L);
+  int cblocks = 1, cbsz = 0;
+  if (!chirp_plan(ctx->nsteps, k, &cblocks, &cbsz) || !uniform_grid(E, k, &e0, &de))
+    return fail(ctx, SC_IVR_EUNSUPPORTED, "chirp-z needs an equally spaced grid, k <= %d and at most %d blocks of %d - k + 1 samples",
+                SCI_CHIRP_L - SCI_CHIRP_MIN_BLOCK + 1, SCI_CHIRP_MAX_BLOCKS, SCI_CHIRP_L);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int rows = ctx->nsteps + 1;
   const long long xstride = round_up_ll(rows, 32);
@@ -553,12 +571,13 @@ sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *zin, long long
   double2 *x = (double2 *)ws;
   double2 *pc = (double2 *)(ws + align_up(sizeof(double2) * (size_t)xstride * (size_t)n, 256));
   double2 *hrow = (double2 *)((char *)pc + align_up(sizeof(double2) * (size_t)rows, 256));
-  double2 *HpT = (double2 *)((char *)hrow + align_up(sizeof(double2) * SCI_CHIRP_L, 256));
-  CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, rows, k, pc, hrow, st));
-  CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, k, nullptr, HpT, 1, st));
+  double2 *HpT = (double2 *)((char *)hrow + align_up(sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256));
+  double2 *yscr = (double2 *)((char *)HpT + align_up(sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256));
+  CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, rows, k, cblocks, cbsz, pc, hrow, st));
+  CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, k, nullptr, HpT, cblocks, cbsz, nullptr, 1, st));
   CU(sci_launch_rows_from_z((const double2 *)zin, n, rows, pc, x, xstride, st));
   const int grid = n < ctx->sm_count ? (int)n : ctx->sm_count;
-  CU(sci_launch_chirp_fft(2, x, xstride, rows, n, HpT, nullptr, k, k, P_out, nullptr, grid, st));
+  CU(sci_launch_chirp_fft(2, x, xstride, rows, n, HpT, nullptr, k, k, P_out, nullptr, cblocks, cbsz, yscr, grid, st));
   return SC_IVR_OK;
 }
 

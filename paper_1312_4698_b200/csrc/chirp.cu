@@ -4,8 +4,9 @@
 // is a chirp-z transform.  With theta = dE dt and  i c = (i^2 + c^2 - (i - c)^2) / 2,
 //     A_i = exp(i theta i^2 / 2) * sum_c [ z_c exp(i (E_0 dt c + theta c^2 / 2)) ] * exp(-i theta (i - c)^2 / 2)
 //         = exp(i theta i^2 / 2) * (x * h)_i,      x_c = z_c pc_c,   h_m = exp(-i theta m^2 / 2),  m = -n .. k-1,
-// a linear convolution, evaluated exactly (to rounding) as a circular one of length L = 8192 >= n + k with two FFTs per
-// trajectory.  Only |A_i|^2 = |(x * h)_i|^2 enters I(E) (Eq. 11), so the outer chirp is never applied.
+// a linear convolution, evaluated exactly (to rounding) as a circular one of length L = 8192 with two FFTs per block of
+// B = L - k + 1 time samples (one block when n + k <= L; longer series are split, block b using the filter shifted by
+// its offset, h^(b)_m = h_(m - b B), and the blocks' outputs y^(b) are added before the modulus is taken).  Only |A_i|^2 = |(x * h)_i|^2 enters I(E) (Eq. 11), so the outer chirp is never applied.
 // Cost per trajectory-step: ~ 2 * 5 L log2 L / (n + 1) = 270 flop instead of 8 k = 32000 for the direct sum.
 //
 // One CTA transforms one trajectory at a time out of shared memory (L complex doubles = 128 KB + padding) and loops
@@ -145,7 +146,8 @@ __device__ __forceinline__ void powers16(double2 w, double2 (&tw)[16]) {
 template <int MODE>
 __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__ x, long long xstride, int n1, long long nrows,
                                                      const double2 *__restrict__ HpT, const double *__restrict__ wg, int k,
-                                                     int kp, double *__restrict__ out, double2 *__restrict__ spec_out) {
+                                                     int kp, double *__restrict__ out, double2 *__restrict__ spec_out,
+                                                     int nblocks, int bsz, double2 *__restrict__ yscr) {
   extern __shared__ double2 S[];
   const int t = threadIdx.x;
   // per-thread base twiddles (fixed for the whole launch): W_L^t, W_L^(t+256), W_512^(t & 31)
@@ -165,8 +167,12 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
 #pragma unroll
     for (int s = 0; s < 16; s++) acc[b][s] = 0.0;
 
-  for (long long row = blockIdx.x; row < nrows; row += gridDim.x) {
-    const double2 *xr = x + row * xstride;
+  double2 *ys = (nblocks > 1) ? yscr + (long long)blockIdx.x * CL : nullptr;  // this CTA's running sum of block outputs
+  for (long long row = blockIdx.x; row < nrows; row += gridDim.x)
+  for (int blk = 0; blk < nblocks; blk++) {
+    const double2 *xr = x + row * xstride + (long long)blk * bsz;
+    const int n1b = min(bsz, n1 - blk * bsz);
+    const double2 *Hb = HpT + (long long)blk * CL;
     // ---- forward pass 1: radix 16 over stride 512, input from HBM (zero beyond n1), twiddle W_L^(n' k1)
 #pragma unroll
     for (int b = 0; b < 2; b++) {
@@ -175,7 +181,7 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
 #pragma unroll
       for (int j = 0; j < 16; j++) {
         const int idx = np + 512 * j;
-        v[j] = (idx < n1) ? xr[idx] : make_double2(0.0, 0.0);
+        v[j] = (idx < n1b) ? xr[idx] : make_double2(0.0, 0.0);
       }
       dft_reg<16, false>(v);
       double2 tw[16];
@@ -218,7 +224,7 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
         for (int s = 0; s < 32; s++) spec_out[s * CT + t] = make_double2(v[s].x * sc, v[s].y * sc);
       } else {
 #pragma unroll
-        for (int s = 0; s < 32; s++) v[s] = cmul(v[s], HpT[s * CT + t]);
+        for (int s = 0; s < 32; s++) v[s] = cmul(v[s], Hb[s * CT + t]);
         dft_reg_dit<32, true>(v);  // bit-reversed spectrum in, natural n'' out
 #pragma unroll
         for (int j = 0; j < 32; j++) S[phys(t * 32 + j)] = v[j];
@@ -262,6 +268,17 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
 #pragma unroll
       for (int s = 0; s < 16; s++) {
         const int i = np + 512 * brev<16>(s);
+        if (nblocks > 1) {  // y = sum of the blocks' outputs, kept in this CTA's global scratch row between blocks
+          if (i < kp) {
+            if (blk > 0) {
+              const double2 p = ys[i];
+              v[s].x += p.x;
+              v[s].y += p.y;
+            }
+            if (blk < nblocks - 1) ys[i] = v[s];
+          }
+          if (blk < nblocks - 1) continue;
+        }
         const double m = fma(v[s].x, v[s].x, v[s].y * v[s].y);
         if (MODE == 0) {
           acc[b][s] += (w != 0.0) ? w * m : 0.0;  // a rejected trajectory may carry NaN: select, never multiply
@@ -283,9 +300,11 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
   }
 }
 
-// pc[c] = exp(i (E_0 dt c + theta c^2 / 2)), c = 0..n1-1, and the filter row hrow[(m + L) % L] = exp(-i theta m^2 / 2)
-// for m = -(n1-1) .. k-1 (zero elsewhere).  c^2 and m^2 are exact in double; the phase carries one rounding.
-__global__ void k_chirp_tables(double e0dt, double theta, int n1, int k, double2 *__restrict__ pc, double2 *__restrict__ hrow) {
+// pc[c] = exp(i (E_0 dt c + theta c^2 / 2)), c = 0..n1-1, and for each block b (offset c0 = b bsz) the filter row
+// hrow[b][(m + L) % L] = exp(-i theta (m - c0)^2 / 2), m = -(bsz-1) .. k-1 (zero elsewhere).  c^2 and (m - c0)^2 are exact
+// in double; the phase carries one rounding.
+__global__ void k_chirp_tables(double e0dt, double theta, int n1, int k, int nblocks, int bsz, double2 *__restrict__ pc,
+                               double2 *__restrict__ hrow) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n1) {
     const double c = (double)i;
@@ -296,18 +315,20 @@ __global__ void k_chirp_tables(double e0dt, double theta, int n1, int k, double2
   if (i < CL) {
     int m = i;
     bool in = (m <= k - 1);
-    if (!in && i >= CL - (n1 - 1)) {
+    if (!in && i >= CL - (bsz - 1)) {
       m = i - CL;
       in = true;
     }
-    double2 v = make_double2(0.0, 0.0);
-    if (in) {
-      const double mm = (double)m;
-      double s, co;
-      sincos(-0.5 * theta * (mm * mm), &s, &co);
-      v = make_double2(co, s);
+    for (int b = 0; b < nblocks; b++) {
+      double2 v = make_double2(0.0, 0.0);
+      if (in) {
+        const double mm = (double)(m - b * bsz);
+        double s, co;
+        sincos(-0.5 * theta * (mm * mm), &s, &co);
+        v = make_double2(co, s);
+      }
+      hrow[(long long)b * CL + i] = v;
     }
-    hrow[i] = v;
   }
 }
 
@@ -376,9 +397,10 @@ __global__ void k_rows_from_z(const double2 *__restrict__ z, long long n, int n1
 size_t sci_chirp_smem_bytes() { return sizeof(double2) * CPAD; }
 int sci_chirp_threads() { return CT; }
 
-cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, double2 *pc, double2 *hrow, cudaStream_t st) {
+cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, int nblocks, int bsz, double2 *pc, double2 *hrow,
+                                    cudaStream_t st) {
   const int n = n1 > CL ? n1 : CL;
-  k_chirp_tables<<<(n + 255) / 256, 256, 0, st>>>(e0dt, theta, n1, k, pc, hrow);
+  k_chirp_tables<<<(n + 255) / 256, 256, 0, st>>>(e0dt, theta, n1, k, nblocks, bsz, pc, hrow);
   return cudaGetLastError();
 }
 
@@ -389,9 +411,11 @@ cudaError_t sci_launch_zassemble_rows(const double4 *raw, long long raw_stride, 
   return cudaGetLastError();
 }
 
-// mode 0: partial spectra (out = partial [grid][kp]); mode 1: filter spectrum (spec_out [8192]); mode 2: per-row power (out [nrows][k])
+// mode 0: partial spectra (out = partial [grid][kp]); mode 1: filter spectra of the nblocks rows of x (spec_out [nblocks][8192]);
+// mode 2: per-row power (out [nrows][k]).  yscr: [grid][8192] complex scratch, needed when nblocks > 1.
 cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, int n1, long long nrows, const double2 *HpT,
-                                 const double *wg, int k, int kp, double *out, double2 *spec_out, int grid, cudaStream_t st) {
+                                 const double *wg, int k, int kp, double *out, double2 *spec_out, int nblocks, int bsz,
+                                 double2 *yscr, int grid, cudaStream_t st) {
   const size_t smem = sci_chirp_smem_bytes();
   static bool attr_set = false;
   if (!attr_set) {
@@ -401,9 +425,15 @@ cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, 
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  if (mode == 0) k_chirp_fft<0><<<grid, CT, smem, st>>>(x, xstride, n1, nrows, HpT, wg, k, kp, out, spec_out);
-  else if (mode == 1) k_chirp_fft<1><<<1, CT, smem, st>>>(x, xstride, n1, 1, HpT, wg, k, kp, out, spec_out);
-  else k_chirp_fft<2><<<grid, CT, smem, st>>>(x, xstride, n1, nrows, HpT, wg, k, kp, out, spec_out);
+  if (mode == 0) {
+    k_chirp_fft<0><<<grid, CT, smem, st>>>(x, xstride, n1, nrows, HpT, wg, k, kp, out, spec_out, nblocks, bsz, yscr);
+  } else if (mode == 1) {
+    for (int b = 0; b < nblocks; b++)  // one full-length row per block
+      k_chirp_fft<1><<<1, CT, smem, st>>>(x + (long long)b * CL, CL, CL, 1, HpT, wg, k, kp, out, spec_out + (long long)b * CL, 1,
+                                          CL, nullptr);
+  } else {
+    k_chirp_fft<2><<<grid, CT, smem, st>>>(x, xstride, n1, nrows, HpT, wg, k, kp, out, spec_out, nblocks, bsz, yscr);
+  }
   return cudaGetLastError();
 }
 

@@ -83,12 +83,16 @@ cudaError_t sci_launch_final(const double *partial, long long ntiles, int kp, in
 cudaError_t sci_fp64_probe(int mode, int iters, double *flops, double *ms);
 
 // chirp-z Fourier stage for equally spaced energy grids (chirp.cu)
-#define SCI_CHIRP_L 8192  // circular convolution length: the fast path needs (nsteps + 1) + k - 1 <= SCI_CHIRP_L
+#define SCI_CHIRP_L 8192        // circular convolution length; blocks of SCI_CHIRP_L - k + 1 time samples
+#define SCI_CHIRP_MIN_BLOCK 1024 // shorter blocks (k > 7169) or more than SCI_CHIRP_MAX_BLOCKS of them: direct sum instead
+#define SCI_CHIRP_MAX_BLOCKS 16
 size_t sci_chirp_smem_bytes();
-cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, double2 *pc, double2 *hrow, cudaStream_t st);
+cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, int nblocks, int bsz, double2 *pc, double2 *hrow,
+                                    cudaStream_t st);
 cudaError_t sci_launch_zassemble_rows(const double4 *raw, long long raw_stride, long long nb, int nsteps, const double2 *pc,
                                       double2 *xrows, long long xstride, cudaStream_t st);
 cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const double2 *pc, double2 *xrows, long long xstride,
                                    cudaStream_t st);
 cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, int n1, long long nrows, const double2 *HpT,
-                                 const double *wg, int k, int kp, double *out, double2 *spec_out, int grid, cudaStream_t st);
+                                 const double *wg, int k, int kp, double *out, double2 *spec_out, int nblocks, int bsz,
+                                 double2 *yscr, int grid, cudaStream_t st);

@@ -150,10 +150,12 @@ def test_fourier_parity(torch_cuda, B, oracle):
 
 @pytest.mark.parametrize("nsteps,n,k,emin,emax", [(333, 150, 70, 0.0, 20000.0), (4000, 37, 4000, 0.0, 20000.0),
                                                  (4191, 5, 4000, 1500.0, 9000.0), (1, 3, 1, 700.0, 700.0),
-                                                 (2999, 9, 2000, -3000.0, 20000.0)])
+                                                 (2999, 9, 2000, -3000.0, 20000.0), (8000, 7, 4000, 0.0, 20000.0),
+                                                 (5000, 3, 7000, 100.0, 30000.0)])
 def test_fourier_chirp_z_parity(torch_cuda, B, oracle, nsteps, n, k, emin, emax):
     """a8 on an equally spaced grid: |A_j(E_i)|^2 from the chirp-z (FFT) kernels vs the definition
-    (one cexp per term) in the oracle; sizes up to the limit nsteps + k = 8191 + 1, grids that do not start at 0."""
+    (one cexp per term) in the oracle; one block up to nsteps + k = 8191 + 1, longer series in several blocks (8000 steps:
+    2 blocks of 4193, k = 7000: 5 blocks of 1193), grids that do not start at 0."""
     torch = torch_cuda
     rng = np.random.default_rng(11)
     w = inputs.make_config(1, ntraj=2, nsteps=nsteps, k=k)
@@ -187,6 +189,17 @@ def test_run_fourier_paths_agree_with_oracle(torch_cuda, B, oracle, mode):
     if mode == "direct_nonuniform_grid":
         w.E = w.E + 1e-7 * np.sin(np.arange(w.k))  # breaks equal spacing far beyond rounding
     ctx = B.ScIvr.from_workload(w, fourier_mode=1 if mode == "direct_forced" else 0)
+    I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
+    Io, ngo, rco = oracle.run_workload(w)
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I.cpu().numpy(), Io)
+
+
+def test_run_long_series_takes_the_blocked_chirp_path(torch_cuda, B, oracle):
+    """nsteps + k > 8192: the chirp-z stage splits the time series into blocks (config 5's 8000-step shape, scaled)."""
+    torch = torch_cuda
+    w = inputs.make_config(5, ntraj=48, nsteps=6000, k=4000)
+    ctx = B.ScIvr.from_workload(w)
     I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
     Io, ngo, rco = oracle.run_workload(w)
     assert (ng, rc) == (ngo, rco)
