@@ -156,6 +156,17 @@ bool chirp_applies(const sc_ivr_ctx *ctx, const double *E, int k, double *e0, do
   return uniform_grid(E, k, e0, de);
 }
 
+// kernel A: one thread per trajectory for F <= SCI_TPT_MAXF, F lanes per trajectory above
+cudaError_t launch_kernel_a(const sc_ivr_ctx *ctx, const PropParams &P, cudaStream_t st) {
+  if (ctx->F <= SCI_TPT_MAXF) {
+    TptParams TP;
+    TP.P = P;
+    memcpy(TP.coef, ctx->tpt_coef, sizeof(TP.coef));
+    return sci_tpt_launch_propagate(ctx->F, ctx->kind, TP, st);
+  }
+  return sci_launch_propagate(ctx->F, ctx->kind, P, st);
+}
+
 struct StageTimer {
   sc_ivr_ctx *ctx;
   cudaStream_t st;
@@ -275,7 +286,13 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
       rc = fail(nullptr, SC_IVR_ECUDA, "coefficient upload: %s", cudaGetErrorString(ce));
       break;
     }
-    ctx->wave = (long long)ctx->sm_count * sci_prop_blocks_per_sm(F, (int)kind) * sci_prop_traj_per_block(F);
+    if (F <= SCI_TPT_MAXF) {  // one thread per trajectory
+      memset(ctx->tpt_coef, 0, sizeof(ctx->tpt_coef));
+      sci_tpt_pack_coeffs(F, (int)kind, pes_coeffs, gamma, ctx->tpt_coef);
+      ctx->wave = (long long)ctx->sm_count * sci_tpt_blocks_per_sm(F, (int)kind) * sci_tpt_traj_per_block();
+    } else {
+      ctx->wave = (long long)ctx->sm_count * sci_prop_blocks_per_sm(F, (int)kind) * sci_prop_traj_per_block(F);
+    }
   } while (0);
   if (rc != SC_IVR_OK) {
     sc_ivr_destroy(ctx);
@@ -405,7 +422,7 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
     P.nb = nb;
     P.good = good + j0;
     tm.begin();
-    CU(sci_launch_propagate(F, ctx->kind, P, st));
+    CU(launch_kernel_a(ctx, P, st));
     tm.end(0);
     tm.begin();
     if (chirp) CU(sci_launch_zassemble_rows(raw, cv.nbatch, nb, ctx->nsteps, pc, z, cv.xstride, st));
@@ -499,7 +516,7 @@ sc_ivr_status sc_ivr_propagate(sc_ivr_ctx *ctx, const double *p0q0, long long nt
   P.pq_out = pq_out;
   P.S_out = S_out;
   P.M_out = M_out;
-  CU(sci_launch_propagate(ctx->F, ctx->kind, P, st));
+  CU(launch_kernel_a(ctx, P, st));
   if (need_raw)
     CU(sci_launch_zassemble((const double4 *)workspace, ntraj, ntraj, nsteps_run, (double2 *)z_out, ntraj, ntraj, nsteps_run + 1,
                             theta_out, st));
@@ -511,6 +528,13 @@ sc_ivr_status sc_ivr_eval_pes(sc_ivr_ctx *ctx, const double *q, long long n, dou
   if (!ctx) return SC_IVR_EINVAL;
   if (!q || !V_out || !g_out || !H_out) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (n < 1) return fail(ctx, SC_IVR_EINVAL, "n must be >= 1");
+  if (ctx->F <= SCI_TPT_MAXF) {
+    TptParams TP;
+    fill_prop_params(ctx, TP.P, nullptr);
+    memcpy(TP.coef, ctx->tpt_coef, sizeof(TP.coef));
+    CU(sci_tpt_launch_eval_pes(ctx->F, ctx->kind, TP, q, n, V_out, g_out, H_out, (cudaStream_t)cuda_stream));
+    return SC_IVR_OK;
+  }
   CU(sci_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
                          (cudaStream_t)cuda_stream));
   return SC_IVR_OK;

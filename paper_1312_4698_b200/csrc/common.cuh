@@ -39,6 +39,15 @@ struct PropParams {
   double *pq_out, *S_out, *M_out;
 };
 
+// thread-per-trajectory kernels (F <= SCI_TPT_MAXF, propagate_tpt.cu): parameters + dense reduced PES constants, all
+// passed by value so that the constants are constant-bank operands
+#define SCI_TPT_MAXF 3
+#define SCI_TPT_NCOEF 40
+struct TptParams {
+  PropParams P;
+  double coef[SCI_TPT_NCOEF];
+};
+
 struct sc_ivr_ctx {
   int F, kind, nsteps, det_stride, integrator, fourier_mode;
   double dt, det_tol, lu_growth_max;
@@ -47,6 +56,7 @@ struct sc_ivr_ctx {
   double sa[SCI_MAX_STAGES], sb[SCI_MAX_STAGES];
   double *d_coef;
   size_t n_coef;
+  double tpt_coef[SCI_TPT_NCOEF];  // F <= SCI_TPT_MAXF only
   int device, sm_count;
   long long wave;  // trajectories one full wave of kernel A holds (batch granularity)
   char err[512];
@@ -65,6 +75,14 @@ size_t sci_pack_coeffs(int F, int kind, const double *coeffs, const double *gamm
 cudaError_t sci_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st);
 cudaError_t sci_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q,
                                 long long n, double *V, double *g, double *H, cudaStream_t st);
+
+// thread-per-trajectory kernels (propagate_tpt.cu)
+int sci_tpt_traj_per_block();
+int sci_tpt_blocks_per_sm(int F, int kind);
+int sci_tpt_pack_coeffs(int F, int kind, const double *coeffs, const double *gamma, double *out /*[SCI_TPT_NCOEF]*/);
+cudaError_t sci_tpt_launch_propagate(int F, int kind, const TptParams &TP, cudaStream_t st);
+cudaError_t sci_tpt_launch_eval_pes(int F, int kind, const TptParams &TP, const double *q, long long n, double *V, double *g,
+                                    double *H, cudaStream_t st);
 
 // spectrum stage (spectrum.cu)
 #define SCI_TJ 128  // trajectories per Fourier tile
