@@ -349,30 +349,41 @@ __global__ void __launch_bounds__(64) k_zassemble_rows(const double4 *__restrict
   const int n1 = nsteps + 1;
   for (int c0 = 0; c0 < n1; c0 += 32) {
     const int cn = min(32, n1 - c0);
-    for (int cc = 0; cc < cn; cc++) {
-      const int c = c0 + cc;
-      const double4 r = raw[(long long)c * raw_stride + jr];
-      const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
-      const double x = r.z * inv, y = r.w * inv;
-      double ur, ui;
-      if (x >= 0.0) {
-        ur = sqrt(0.5 * (1.0 + x));
-        ui = 0.5 * y / ur;
-      } else {
-        ui = copysign(sqrt(0.5 * (1.0 - x)), y);
-        ur = 0.5 * y / ui;
+    for (int cb = 0; cb < cn; cb += 8) {
+      // eight independent record loads in flight before the (sequential) branch rule consumes them
+      double4 rec[8];
+#pragma unroll
+      for (int u = 0; u < 8; u++) {
+        const int c = min(c0 + cb + u, nsteps);
+        rec[u] = raw[(long long)c * raw_stride + jr];
       }
-      if (ur * upr + ui * upi < 0.0) {
-        ur = -ur;
-        ui = -ui;
+#pragma unroll
+      for (int u = 0; u < 8; u++) {
+        const int cc = cb + u, c = c0 + cc;
+        if (cc >= cn) break;
+        const double4 r = rec[u];
+        const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
+        const double x = r.z * inv, y = r.w * inv;
+        double ur, ui;
+        if (x >= 0.0) {
+          ur = sqrt(0.5 * (1.0 + x));
+          ui = 0.5 * y / ur;
+        } else {
+          ui = copysign(sqrt(0.5 * (1.0 - x)), y);
+          ur = 0.5 * y / ui;
+        }
+        if (ur * upr + ui * upi < 0.0) {
+          ur = -ur;
+          ui = -ui;
+        }
+        upr = ur;
+        upi = ui;
+        const double ea = exp(r.x);
+        double s, co;
+        sincos(r.y, &s, &co);
+        const double2 z = make_double2(ea * (co * ur - s * ui), ea * (co * ui + s * ur));
+        tile[warp][lane][cc] = cmul(z, pc[c]);
       }
-      upr = ur;
-      upi = ui;
-      const double ea = exp(r.x);
-      double s, co;
-      sincos(r.y, &s, &co);
-      const double2 z = make_double2(ea * (co * ur - s * ui), ea * (co * ui + s * ur));
-      tile[warp][lane][cc] = cmul(z, pc[c]);
     }
     __syncwarp();
     for (int rr = 0; rr < 32; rr++) {
