@@ -13,7 +13,7 @@
 // over its trajectories (persistent, fixed assignment => fixed summation order, no atomics):
 //   forward  DIF passes of radix 16, 16, 32 (natural order in, digit-reversed out; pass 1 reads x from HBM),
 //   pointwise product with the filter spectrum Hp (stored in the same digit-reversed order, 1/L folded in),
-//   inverse  DIT passes of radix 32, 16, 16 (digit-reversed in, natural out), |y_i|^2 w_j accumulated in registers.
+//   inverse  DIT passes of radix 32, 16, 16 (digit-reversed in, natural out), |y_i|^2 w_j accumulated in shared memory.
 // The radix-32 forward pass, the product and the radix-32 inverse pass run on registers without touching memory.
 #include "common.cuh"
 
@@ -161,11 +161,11 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
     sincospi(-2.0 * (double)(t & 31) / 512.0, &s, &c);
     w2 = make_double2(c, s);
   }
-  double acc[2][16];
-#pragma unroll
-  for (int b = 0; b < 2; b++)
-#pragma unroll
-    for (int s = 0; s < 16; s++) acc[b][s] = 0.0;
+  // power accumulators of this CTA, one per output i < kp, behind the FFT buffer in shared memory (thread t owns
+  // i = t + 256 b + 512 j: no two threads share an entry, consecutive threads hit consecutive banks)
+  double *accs = reinterpret_cast<double *>(S + CPAD);
+  if (MODE == 0)
+    for (int i = t; i < CL; i += CT) accs[i] = 0.0;
 
   double2 *ys = (nblocks > 1) ? yscr + (long long)blockIdx.x * CL : nullptr;  // this CTA's running sum of block outputs
   for (long long row = blockIdx.x; row < nrows; row += gridDim.x)
@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
         }
         const double m = fma(v[s].x, v[s].x, v[s].y * v[s].y);
         if (MODE == 0) {
-          acc[b][s] += (w != 0.0) ? w * m : 0.0;  // a rejected trajectory may carry NaN: select, never multiply
+          if (i < kp && w != 0.0) accs[i] = fma(w, m, accs[i]);  // a rejected trajectory may carry NaN: skip, never multiply
         } else if (i < k) {
           out[row * (long long)k + i] = m;
         }
@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(CT, 1) k_chirp_fft(const double2 *__restrict__
 #pragma unroll
       for (int s = 0; s < 16; s++) {
         const int i = t + 256 * b + 512 * brev<16>(s);
-        if (i < kp) out[(long long)blockIdx.x * kp + i] = acc[b][s];
+        if (i < kp) out[(long long)blockIdx.x * kp + i] = accs[i];
       }
   }
 }
@@ -336,7 +336,13 @@ __global__ void k_chirp_tables(double e0dt, double theta, int n1, int k, int nbl
 // inner chirp pc[c]; output x[j][c] with the time series of a trajectory contiguous.  One warp = 32 trajectories; the
 // records are read time-major (coalesced over trajectories), transposed through a padded shared tile and written as
 // 512-byte row segments.
-__global__ void __launch_bounds__(64) k_zassemble_rows(const double4 *__restrict__ raw, long long raw_stride, long long nb, int nsteps,
+#ifndef SCI_ZU
+#define SCI_ZU 4
+#endif
+#ifndef SCI_ZREG
+#define SCI_ZREG 128
+#endif
+__global__ void __maxnreg__(SCI_ZREG) k_zassemble_rows(const double4 *__restrict__ raw, long long raw_stride, long long nb, int nsteps,
                                                         const double2 *__restrict__ pc, double2 *__restrict__ xrows, long long xstride) {
   __shared__ double2 tile[2][32][33];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -349,16 +355,16 @@ __global__ void __launch_bounds__(64) k_zassemble_rows(const double4 *__restrict
   const int n1 = nsteps + 1;
   for (int c0 = 0; c0 < n1; c0 += 32) {
     const int cn = min(32, n1 - c0);
-    for (int cb = 0; cb < cn; cb += 8) {
-      // eight independent record loads in flight before the (sequential) branch rule consumes them
-      double4 rec[8];
+    for (int cb = 0; cb < cn; cb += SCI_ZU) {
+      // SCI_ZU independent record loads in flight before the (sequential) branch rule consumes them
+      double4 rec[SCI_ZU];
 #pragma unroll
-      for (int u = 0; u < 8; u++) {
+      for (int u = 0; u < SCI_ZU; u++) {
         const int c = min(c0 + cb + u, nsteps);
         rec[u] = raw[(long long)c * raw_stride + jr];
       }
 #pragma unroll
-      for (int u = 0; u < 8; u++) {
+      for (int u = 0; u < SCI_ZU; u++) {
         const int cc = cb + u, c = c0 + cc;
         if (cc >= cn) break;
         const double4 r = rec[u];
@@ -405,7 +411,7 @@ __global__ void k_rows_from_z(const double2 *__restrict__ z, long long n, int n1
 
 }  // namespace
 
-size_t sci_chirp_smem_bytes() { return sizeof(double2) * CPAD; }
+size_t sci_chirp_smem_bytes() { return sizeof(double2) * CPAD + sizeof(double) * CL; }
 int sci_chirp_threads() { return CT; }
 
 cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, int nblocks, int bsz, double2 *pc, double2 *hrow,
