@@ -164,3 +164,33 @@ def spectrum(pes, gamma, dt, nsteps, p0q0, chi, E, weights=None, det_tol=1e-6, s
         return np.zeros(E.size), 0, A_all
     T = nsteps * dt
     return I * dt ** 2 / ((2 * np.pi) ** (F + 1) * T * n_good), n_good, A_all
+
+
+def spectrum_combo(pes, gamma, dt, nsteps, p0q0, chis, eps, E, scheme=VV):
+    """Eq. 11 by the definition for the reference state |chi> = sum_m eps[m] |p_m, q_m>:
+    <chi|p q> = sum_m conj(eps[m]) <p_m q_m|p q>, each overlap from Eq. 3 in closed form.  Returns (I [k], n_good)."""
+    F = pes.F
+    gamma = np.asarray(gamma, dtype=np.float64)
+    p0q0 = np.asarray(p0q0, dtype=np.float64).reshape(2 * F, -1)
+    chis = np.asarray(chis, dtype=np.float64).reshape(-1, 2 * F)
+    eps = np.asarray(eps, dtype=np.complex128).reshape(-1)
+    E = np.asarray(E, dtype=np.float64)
+    tw = np.exp(1j * np.outer(np.arange(nsteps + 1) * dt, E))
+    I = np.zeros(E.size)
+    n_good = 0
+    for j in range(p0q0.shape[1]):
+        t = trajectory(pes, gamma, dt, nsteps, p0q0[:F, j], p0q0[F:, j], chis[0], scheme)
+        ovl = np.zeros(nsteps + 1, dtype=np.complex128)
+        for m in range(chis.shape[0]):
+            dq = chis[m, F:][None, :] - t["q"]
+            dp = chis[m, :F][None, :] - t["p"]
+            a = np.sum(-0.25 * gamma * dq ** 2 - dp ** 2 / (4 * gamma), axis=1)
+            b = 0.5 * np.sum((chis[m, :F][None, :] + t["p"]) * dq, axis=1)
+            ovl += np.conj(eps[m]) * np.exp(a + 1j * b)
+        z = ovl * np.exp(1j * (t["S"] + t["phi"]))
+        if np.all(np.isfinite(z)) and np.all(np.abs(t["detM"] - 1.0) <= 1e-6):
+            n_good += 1
+            I += np.abs(z @ tw) ** 2
+    if n_good == 0:
+        return np.zeros(E.size), 0
+    return I * dt ** 2 / ((2 * np.pi) ** (F + 1) * nsteps * dt * n_good), n_good

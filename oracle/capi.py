@@ -46,6 +46,10 @@ def lib():
         _lib.sc_ivr_oracle_run.argtypes = [
             C.c_int, C.c_int, _dp, C.c_long, _dp, C.c_double, C.c_int, C.c_int, C.c_int, C.c_double,
             _dp, _dp, C.c_long, _dp, _dp, C.c_int, C.c_int, _dp, C.POINTER(C.c_longlong)]
+        _lib.sc_ivr_oracle_run_combo.restype = C.c_int
+        _lib.sc_ivr_oracle_run_combo.argtypes = [
+            C.c_int, C.c_int, _dp, C.c_long, _dp, C.c_double, C.c_int, C.c_int, C.c_int, C.c_double,
+            _dp, _dp, C.c_long, _dp, C.c_int, _dp, _dp, C.c_int, C.c_int, _dp, C.POINTER(C.c_longlong)]
     return _lib
 
 
@@ -133,6 +137,30 @@ def run(F, kind, coeffs, gamma, dt, nsteps, p0q0, chi, E, weights=None, integrat
         float(det_tol), _p(p0q0), _p(w), n, _p(chi), _p(E), E.size, int(fourier_mode), _p(I), C.byref(ng))
     if rc not in (0, 5):
         raise ValueError(f"oracle run rc={rc}")
+    return I, int(ng.value), rc
+
+
+def run_combo(F, kind, coeffs, gamma, dt, nsteps, p0q0, chis, eps, E, weights=None, integrator=0, det_stride=1,
+              det_tol=1e-6, fourier_mode=1):
+    """The whole path for the reference state |chi> = sum_m eps[m] |chis[m]>.
+    chis [ncs][2F] (p_m then q_m), eps [ncs] complex.  Returns (I [k], n_good, rc)."""
+    coeffs = _f64(coeffs)
+    gamma = _f64(gamma)
+    p0q0 = _f64(p0q0).reshape(2 * F, -1)
+    n = p0q0.shape[1]
+    chis = _f64(chis).reshape(-1, 2 * F)
+    ncs = chis.shape[0]
+    e = np.asarray(eps, dtype=np.complex128).reshape(ncs)
+    ee = np.ascontiguousarray(np.stack([e.real, e.imag], axis=1))
+    E = _f64(E)
+    w = None if weights is None else _f64(weights)
+    I = np.empty(E.size)
+    ng = C.c_longlong(0)
+    rc = lib().sc_ivr_oracle_run_combo(
+        F, kind, _p(coeffs), coeffs.size, _p(gamma), float(dt), int(nsteps), int(integrator), int(det_stride),
+        float(det_tol), _p(p0q0), _p(w), n, _p(chis), ncs, _p(ee), _p(E), E.size, int(fourier_mode), _p(I), C.byref(ng))
+    if rc not in (0, 5):
+        raise ValueError(f"oracle run_combo rc={rc}")
     return I, int(ng.value), rc
 
 

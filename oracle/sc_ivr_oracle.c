@@ -317,6 +317,17 @@ static double complex overlap(const state_t *s, const double *gamma, const doubl
   return exp(a) * cexp(I * b);
 }
 
+/* Reference state as a combination of coherent states, |chi> = sum_m eps_m |p_m, q_m>  (Fig. 4: "different
+ * coherent state combinations for the same irreducible representation"):  <chi|p q> = sum_m conj(eps_m) <p_m q_m|p q>.
+ * chi: [ncs][2F], eps: [ncs][2] (re, im); eps == NULL is the single coherent state chi[0] of PAPER.md:80. */
+static double complex reference_overlap(const state_t *s, const double *gamma, const double *chi, int ncs, const double *eps) {
+  if (!eps) return overlap(s, gamma, chi);
+  double complex sum = 0.0;
+  for (int m = 0; m < ncs; m++)
+    sum += (eps[2 * m] - I * eps[2 * m + 1]) * overlap(s, gamma, chi + 2 * (size_t)s->F * m);
+  return sum;
+}
+
 static double wrap_pi(double x) { /* to (-pi, pi] */
   while (x > M_PI) x -= 2.0 * M_PI;
   while (x <= -M_PI) x += 2.0 * M_PI;
@@ -331,7 +342,7 @@ static double wrap_pi(double x) { /* to (-pi, pi] */
  *   iii. overlap;  iv. z_c = <chi|p q> e^{i S} u;  v. quality flag;  vi. time step.
  * z (may be NULL): [nsteps+1][2].  Returns good flag.
  */
-static int propagate_one(const pes_t *P, const scheme_t *sc, const double *gamma, const double *chi,
+static int propagate_one(const pes_t *P, const scheme_t *sc, const double *gamma, const double *chi, int ncs, const double *eps,
                          double dt, int nsteps, int det_stride, double det_tol,
                          const double *p0, const double *q0, double *z, state_t *final, double *theta_out) {
   const int F = P->F;
@@ -353,7 +364,7 @@ static int propagate_one(const pes_t *P, const scheme_t *sc, const double *gamma
     theta += wrap_pi(argD - argD_prev);
     argD_prev = argD;
     if (z) {
-      double complex zc = overlap(&s, gamma, chi) * cexp(I * s.S) * u;
+      double complex zc = reference_overlap(&s, gamma, chi, ncs, eps) * cexp(I * s.S) * u;
       z[2 * c] = creal(zc);
       z[2 * c + 1] = cimag(zc);
     }
@@ -426,7 +437,7 @@ int sc_ivr_oracle_propagate(int F, int kind, const double *coeffs, long ncoef, c
     state_t fin;
     for (int k = 0; k < F; k++) { p0[k] = p0q0[k * ntraj + j]; q0[k] = p0q0[(F + k) * ntraj + j]; }
     double *z = z_out ? z_out + 2 * (size_t)j * (size_t)(nsteps + 1) : NULL;
-    int good = propagate_one(&P, &sc, gamma, chi_use, dt, nsteps, det_stride, det_tol, p0, q0, z, &fin, &th);
+    int good = propagate_one(&P, &sc, gamma, chi_use, 1, NULL, dt, nsteps, det_stride, det_tol, p0, q0, z, &fin, &th);
     if (pq_out)
       for (int k = 0; k < F; k++) { pq_out[k * ntraj + j] = fin.p[k]; pq_out[(F + k) * ntraj + j] = fin.q[k]; }
     if (S_out) S_out[j] = fin.S;
@@ -502,10 +513,10 @@ int sc_ivr_oracle_fourier(const double *z, long n, int nsteps, double dt, const 
  * energies; within an energy the loop over j is sequential and chunks follow one another).
  * weights may be NULL (= 1).  Returns SCO_ENOGOOD with I = 0 when no trajectory survives (R18).
  */
-int sc_ivr_oracle_run(int F, int kind, const double *coeffs, long ncoef, const double *gamma, double dt,
-                      int nsteps, int integrator, int det_stride, double det_tol, const double *p0q0,
-                      const double *weights, long ntraj, const double *chi, const double *E, int k,
-                      int fourier_mode, double *I_out, long long *n_good_out) {
+static int run_impl(int F, int kind, const double *coeffs, long ncoef, const double *gamma, double dt,
+                    int nsteps, int integrator, int det_stride, double det_tol, const double *p0q0,
+                    const double *weights, long ntraj, const double *chi, int ncs, const double *eps, const double *E, int k,
+                    int fourier_mode, double *I_out, long long *n_good_out) {
   pes_t P;
   scheme_t sc;
   int rc = pes_init(&P, F, kind, coeffs, ncoef);
@@ -526,7 +537,7 @@ int sc_ivr_oracle_run(int F, int kind, const double *coeffs, long ncoef, const d
       long j = j0 + jj;
       double p0[SCO_MAXF], q0[SCO_MAXF];
       for (int a = 0; a < F; a++) { p0[a] = p0q0[a * ntraj + j]; q0[a] = p0q0[(F + a) * ntraj + j]; }
-      good[jj] = (unsigned char)propagate_one(&P, &sc, gamma, chi, dt, nsteps, det_stride, det_tol, p0, q0,
+      good[jj] = (unsigned char)propagate_one(&P, &sc, gamma, chi, ncs, eps, dt, nsteps, det_stride, det_tol, p0, q0,
                                               z + 2 * (size_t)jj * (size_t)(nsteps + 1), NULL, NULL);
     }
     for (long jj = 0; jj < nj; jj++) n_good += good[jj];
@@ -557,4 +568,22 @@ int sc_ivr_oracle_run(int F, int kind, const double *coeffs, long ncoef, const d
   double norm = dt * dt / (pow(2.0 * M_PI, F + 1) * T * (double)n_good);
   for (int i = 0; i < k; i++) I_out[i] *= norm;
   return SCO_OK;
+}
+
+int sc_ivr_oracle_run(int F, int kind, const double *coeffs, long ncoef, const double *gamma, double dt,
+                      int nsteps, int integrator, int det_stride, double det_tol, const double *p0q0,
+                      const double *weights, long ntraj, const double *chi, const double *E, int k,
+                      int fourier_mode, double *I_out, long long *n_good_out) {
+  return run_impl(F, kind, coeffs, ncoef, gamma, dt, nsteps, integrator, det_stride, det_tol, p0q0, weights, ntraj, chi, 1, NULL,
+                  E, k, fourier_mode, I_out, n_good_out);
+}
+
+/* The same path with the reference state |chi> = sum_m eps_m |p_m, q_m>  (chi [ncs][2F], eps [ncs][2]): PAPER.md:167-173. */
+int sc_ivr_oracle_run_combo(int F, int kind, const double *coeffs, long ncoef, const double *gamma, double dt,
+                            int nsteps, int integrator, int det_stride, double det_tol, const double *p0q0,
+                            const double *weights, long ntraj, const double *chi, int ncs, const double *eps,
+                            const double *E, int k, int fourier_mode, double *I_out, long long *n_good_out) {
+  if (ncs < 1 || !eps) return SCO_EINVAL;
+  return run_impl(F, kind, coeffs, ncoef, gamma, dt, nsteps, integrator, det_stride, det_tol, p0q0, weights, ntraj, chi, ncs, eps,
+                  E, k, fourier_mode, I_out, n_good_out);
 }

@@ -461,3 +461,46 @@ def test_p12_morse_levels_loose(oracle):
     for l in lev:
         assert min(abs(Ecm[pk] - l)) <= 3 * bin_w
     assert abs(Ecm[np.argmax(I)] - lev[0]) <= 3 * bin_w
+
+
+def test_combo_reference_state_parity_selection_rule(oracle):
+    """Row f4 (Fig. 4): reference state = combination of coherent states.  Closed-form pin: for a
+    1-D harmonic oscillator with gamma = omega, |alpha> + |-alpha> contains only even and |alpha> - |-alpha> only odd
+    number states (the mirror image about q_eq), so each combination keeps every second peak of the single-state
+    spectrum, at (n + 1/2) omega~, and removes the others."""
+    om = 0.01
+    nsteps, dt = 6000, 2.0  # omega dt = 0.02: the Verlet map is harmonic with omega~ = omega (1 + 1.7e-5)
+    E = np.linspace(0.0, 6.0 * om, 601)
+    w = inputs.make_harmonic([om], ntraj=24, nsteps=nsteps, dt=dt, E=E, seed=3)
+    p_e, q_e = w.chi[0], w.chi[1]
+    chis = np.array([[p_e, q_e], [-p_e, -q_e]])  # make_harmonic puts q_eq = 0 unless told otherwise
+    assert abs(q_e) < 1e-15
+    spec = {}
+    for name, eps in (("single", [1.0, 0.0]), ("even", [1.0, 1.0]), ("odd", [1.0, -1.0])):
+        spec[name], ng, rc = oracle.run_combo(1, w.pes_kind, w.pes_coeffs, w.gamma, dt, nsteps, w.p0q0, chis, eps, E,
+                                              fourier_mode=0)
+        assert (ng, rc) == (24, 0)
+    I1, rc1 = oracle.run(1, w.pes_kind, w.pes_coeffs, w.gamma, dt, nsteps, w.p0q0, w.chi, E, fourier_mode=0)[::2]
+    assert np.allclose(spec["single"], I1, rtol=1e-12, atol=0)  # eps = (1, 0) is the plain reference state
+    mx = spec["single"].max()
+    for n in range(5):
+        i = int(round((n + 0.5) * om / (E[1] - E[0])))
+        keep, kill = ("even", "odd") if n % 2 == 0 else ("odd", "even")
+        if spec["single"][i] > 1e-4 * mx:
+            assert spec[kill][i] < 2e-3 * spec["single"][i], (n, spec[kill][i] / spec["single"][i])
+            # amplitude doubles, power x4 (to the side-lobe leakage of the removed neighbours at finite T)
+            assert abs(spec[keep][i] / spec["single"][i] / 4.0 - 1.0) < 3e-2
+
+
+def test_combo_reference_state_brute_force(oracle):
+    """The C oracle against the numpy restatement on a tiny coupled case with complex coefficients and three states."""
+    from oracle import brute
+    w = inputs.make_random_qff(2, 5, 60, 24, seed=21)
+    rng = np.random.default_rng(5)
+    chis = np.stack([w.chi, w.chi * np.array([-1, 1, -1, 1]), w.chi + 0.1 * rng.standard_normal(4)])
+    eps = np.array([1.0, -0.5 + 0.25j, 0.3j])
+    I, ng, rc = oracle.run_combo(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, chis, eps, w.E, fourier_mode=0)
+    pes = brute.make_pes(w.F, w.pes_kind, w.pes_coeffs)
+    Ib, ngb = brute.spectrum_combo(pes, w.gamma, w.dt, w.nsteps, w.p0q0, chis, eps, w.E)
+    assert ng == ngb == 5 and rc == 0
+    assert np.max(np.abs(I - Ib)) < 1e-11 * Ib.max()
