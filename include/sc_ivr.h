@@ -134,6 +134,25 @@ sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double 
                               void *cuda_stream);
 
 /*
+ * Several reference states per run, each a combination of coherent states (Fig. 4: the spectrum is
+ * projected on irreducible representations with "different coherent state combinations"):
+ *   |chi_n> = sum_m eps[n][m] |p_m, q_m>,   <chi_n|p q> = sum_m conj(eps[n][m]) <p_m q_m|p q>   (each overlap: Eq. 3),
+ *   I_out[n][i] = I(E_i) of Eq. 11 with chi = chi_n.
+ * The trajectories (a1-a5, a7) are propagated ONCE and shared by all nchi reference states; only the overlaps (a6) and the
+ * Fourier / reduction stages (a8, a9) are repeated per state.
+ *   chis  HOST [ncs][2F]  (p_m[F] then q_m[F])        eps  HOST [nchi][ncs][2]  (re, im)
+ *   I_out DEVICE [nchi][k]                             E    HOST [k], equally spaced (chirp-z path only)
+ *   workspace DEVICE, sc_ivr_multi_workspace_bytes(ctx, ntraj, k, max_batch); a smaller one (>= one batch of
+ *   sc_ivr_min_batch) makes more, smaller batches.  1 <= ncs <= 16, 1 <= nchi <= 16.
+ * Other arguments, ordering and error behaviour as sc_ivr_run; SC_IVR_EUNSUPPORTED when the grid is not equally spaced or too
+ * long for the chirp-z stage.
+ */
+size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, long long max_batch /*0 = 32768*/);
+sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chis,
+                               int ncs, const double *eps, int nchi, const double *E, int k, double *I_out,
+                               long long *n_good_out, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
  * Parity / debug entry: propagate only (steps a1-a7), return the state after nsteps_run steps
  * (0 <= nsteps_run; independent of the context's nsteps).  Any output may be NULL.
  *   pq_out    DEVICE [2F][ntraj]      S_out  DEVICE [ntraj]       M_out DEVICE [4][F][F][ntraj]

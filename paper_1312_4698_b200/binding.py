@@ -21,7 +21,7 @@ EXPORTS = [
     "sc_ivr_create", "sc_ivr_destroy", "sc_ivr_last_error", "sc_ivr_workspace_bytes", "sc_ivr_min_batch",
     "sc_ivr_run", "sc_ivr_host_staging_bytes", "sc_ivr_run_host", "sc_ivr_propagate_workspace_bytes",
     "sc_ivr_propagate", "sc_ivr_eval_pes", "sc_ivr_fourier_workspace_bytes", "sc_ivr_fourier",
-    "sc_ivr_fourier_power_workspace_bytes", "sc_ivr_fourier_power",
+    "sc_ivr_fourier_power_workspace_bytes", "sc_ivr_fourier_power", "sc_ivr_multi_workspace_bytes", "sc_ivr_run_multi",
     "sc_ivr_fp64_probe", "sc_ivr_set_timing", "sc_ivr_last_timings",
 ]
 
@@ -77,6 +77,11 @@ def lib():
     L.sc_ivr_eval_pes.argtypes = [_vp, _vp, C.c_longlong, _vp, _vp, _vp, _vp]
     L.sc_ivr_fourier_workspace_bytes.restype = C.c_size_t
     L.sc_ivr_fourier_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int]
+    L.sc_ivr_multi_workspace_bytes.restype = C.c_size_t
+    L.sc_ivr_multi_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int, C.c_longlong]
+    L.sc_ivr_run_multi.restype = C.c_int
+    L.sc_ivr_run_multi.argtypes = [_vp, _vp, _vp, C.c_longlong, _dp, C.c_int, _dp, C.c_int, _dp, C.c_int, _vp,
+                                   C.POINTER(C.c_longlong), _vp, C.c_size_t, _vp]
     L.sc_ivr_fourier_power_workspace_bytes.restype = C.c_size_t
     L.sc_ivr_fourier_power_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int]
     L.sc_ivr_fourier_power.restype = C.c_int
@@ -248,6 +253,31 @@ class ScIvr:
         H = torch.empty((F, F, n), dtype=torch.float64, device=dev)
         self._check(lib().sc_ivr_eval_pes(self._h, _dev(q), n, _dev(V), _dev(g), _dev(H), _stream()))
         return V, g, H
+
+    def _lib_multi_bytes(self, ntraj, k, max_batch=0):
+        return int(lib().sc_ivr_multi_workspace_bytes(self._h, int(ntraj), int(k), int(max_batch)))
+
+    def run_multi(self, p0q0, chis, eps, E, weights=None, workspace=None, max_batch=0):
+        """sc_ivr_run_multi: reference states |chi_n> = sum_m eps[n][m] |chis[m]>; p0q0 DEVICE [2F, ntraj];
+        chis [ncs, 2F], eps [nchi, ncs] complex (host) -> (I DEVICE [nchi, k], n_good, status)."""
+        import torch
+        assert p0q0.is_cuda and p0q0.dtype == torch.float64 and p0q0.is_contiguous()
+        ntraj = p0q0.shape[1]
+        chis = _host(np.asarray(chis, dtype=np.float64).reshape(-1, 2 * self.F))
+        ncs = chis.shape[0]
+        e = np.asarray(eps, dtype=np.complex128).reshape(-1, ncs)
+        nchi = e.shape[0]
+        ee = _host(np.stack([e.real, e.imag], axis=2))
+        E = _host(E)
+        I = torch.empty((nchi, E.size), dtype=torch.float64, device=p0q0.device)
+        if workspace is None:
+            workspace = _workspace(lib().sc_ivr_multi_workspace_bytes(self._h, ntraj, E.size, int(max_batch)), p0q0.device)
+        ng = C.c_longlong(0)
+        rc = lib().sc_ivr_run_multi(self._h, _dev(p0q0), _dev(weights) if weights is not None else None, ntraj, _hp(chis), ncs,
+                                    _hp(ee), nchi, _hp(E), E.size, _dev(I), C.byref(ng), _dev(workspace), workspace.numel(),
+                                    _stream())
+        self._check(rc, allow=(5,))
+        return I, int(ng.value), rc
 
     def fourier_power(self, z, E):
         """sc_ivr_fourier_power (chirp-z kernels): z DEVICE complex [nsteps+1, n] -> |A|^2 DEVICE [n, k]."""

@@ -606,3 +606,145 @@ sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *zin, long long
 }
 
 }  // extern "C"
+
+namespace {
+struct CarveMulti {
+  long long nbatch, xstride;
+  int rows, kp;
+  long long tiles_per_chi;  // partial rows per reference state
+  size_t off_raw, off_pq, off_x, off_partial, off_good, off_wg, off_ngood, off_pc, off_hrow, off_HpT, off_yscr, off_chis, off_eps, total;
+};
+CarveMulti carve_multi(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
+  CarveMulti c;
+  c.nbatch = nbatch;
+  c.rows = ctx->nsteps + 1;
+  c.xstride = round_up_ll(c.rows, 32);
+  c.kp = (int)round_up_ll(k, SCI_TI);
+  const long long nbatches = (ntraj + nbatch - 1) / nbatch;
+  c.tiles_per_chi = nbatches * ctx->sm_count;
+  size_t o = 0;
+  c.off_raw = o; o = align_up(o + sizeof(double4) * (size_t)c.rows * (size_t)nbatch, 256);
+  c.off_pq = o; o = align_up(o + sizeof(double2) * (size_t)c.rows * (size_t)ctx->F * (size_t)nbatch, 256);
+  c.off_x = o; o = align_up(o + sizeof(double2) * (size_t)c.xstride * (size_t)nbatch, 256);
+  c.off_partial = o; o = align_up(o + sizeof(double) * 16 * (size_t)c.tiles_per_chi * (size_t)c.kp, 256);
+  c.off_good = o; o = align_up(o + (size_t)ntraj, 256);
+  c.off_wg = o; o = align_up(o + sizeof(double) * (size_t)ntraj, 256);
+  c.off_ngood = o; o = align_up(o + 64, 256);
+  c.off_pc = o; o = align_up(o + sizeof(double2) * (size_t)c.rows, 256);
+  c.off_hrow = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256);
+  c.off_HpT = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L * SCI_CHIRP_MAX_BLOCKS, 256);
+  c.off_yscr = o; o = align_up(o + sizeof(double2) * SCI_CHIRP_L * (size_t)ctx->sm_count, 256);
+  c.off_chis = o; o = align_up(o + sizeof(double) * 16 * 2 * SCI_MAXF, 256);
+  c.off_eps = o; o = align_up(o + sizeof(double) * 16 * 16 * 2, 256);
+  c.total = o;
+  return c;
+}
+}  // namespace
+
+extern "C" {
+
+size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, long long max_batch) {
+  if (!ctx || ntraj < 1 || k < 1) return 0;
+  return carve_multi(ctx, ntraj, k, default_batch(ctx, ntraj, max_batch > 0 ? max_batch : 32768)).total;
+}
+
+sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chis,
+                               int ncs, const double *eps, int nchi, const double *E, int k, double *I_out,
+                               long long *n_good_out, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (!p0q0 || !chis || !eps || !E || !I_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (ntraj < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "ntraj and k must be >= 1");
+  if (ncs < 1 || ncs > 16 || nchi < 1 || nchi > 16) return fail(ctx, SC_IVR_EINVAL, "ncs and nchi must be in 1..16");
+  if (((uintptr_t)workspace & 255) != 0) return fail(ctx, SC_IVR_EINVAL, "workspace must be 256-byte aligned");
+  const int F = ctx->F;
+  for (int i = 0; i < ncs * 2 * F; i++)
+    if (!isfinite(chis[i])) return fail(ctx, SC_IVR_EINVAL, "chis[%d] is not finite", i);
+  for (int i = 0; i < nchi * ncs * 2; i++)
+    if (!isfinite(eps[i])) return fail(ctx, SC_IVR_EINVAL, "eps[%d] is not finite", i);
+  double e0 = 0.0, de = 0.0;
+  int cblocks = 1, cbsz = 0;
+  if (!chirp_plan(ctx->nsteps, k, &cblocks, &cbsz) || !uniform_grid(E, k, &e0, &de))
+    return fail(ctx, SC_IVR_EUNSUPPORTED, "sc_ivr_run_multi needs an equally spaced grid within the chirp-z limits");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+
+  long long nbatch = default_batch(ctx, ntraj, 32768);
+  CarveMulti cv = carve_multi(ctx, ntraj, k, nbatch);
+  while (cv.total > workspace_bytes && nbatch > ctx->wave) {
+    long long nx = nbatch / 2 / ctx->wave * ctx->wave;
+    if (nx < ctx->wave) nx = ctx->wave;
+    nbatch = nx;
+    cv = carve_multi(ctx, ntraj, k, nbatch);
+  }
+  if (cv.total > workspace_bytes)
+    return fail(ctx, SC_IVR_EINVAL, "workspace too small: %zu bytes given, %zu needed for the minimum batch of %lld", workspace_bytes,
+                cv.total, nbatch);
+  char *ws = (char *)workspace;
+  double4 *raw = (double4 *)(ws + cv.off_raw);
+  double2 *pqs = (double2 *)(ws + cv.off_pq);
+  double2 *x = (double2 *)(ws + cv.off_x);
+  double *partial = (double *)(ws + cv.off_partial);
+  unsigned char *good = (unsigned char *)(ws + cv.off_good);
+  double *wg = (double *)(ws + cv.off_wg);
+  long long *ngood = (long long *)(ws + cv.off_ngood);
+  double2 *pc = (double2 *)(ws + cv.off_pc);
+  double2 *hrow = (double2 *)(ws + cv.off_hrow);
+  double2 *HpT = (double2 *)(ws + cv.off_HpT);
+  double2 *yscr = (double2 *)(ws + cv.off_yscr);
+  double *chis_dev = (double *)(ws + cv.off_chis);
+  double *eps_dev = (double *)(ws + cv.off_eps);
+
+  // reference coherent states in reduced coordinates (P_eq then Q_eq per state); the copies are synchronous-safe
+  // because the host arrays below live until the stream is synchronised at the end of this call
+  std::vector<double> chr((size_t)ncs * 2 * F);
+  for (int m = 0; m < ncs; m++)
+    for (int a = 0; a < F; a++) {
+      const double sg = sqrt(ctx->gamma[a]);
+      chr[(size_t)(2 * m) * F + a] = chis[(size_t)m * 2 * F + a] / sg;
+      chr[(size_t)(2 * m + 1) * F + a] = chis[(size_t)m * 2 * F + F + a] * sg;
+    }
+  CU(cudaMemcpyAsync(chis_dev, chr.data(), sizeof(double) * chr.size(), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(eps_dev, eps, sizeof(double) * (size_t)nchi * ncs * 2, cudaMemcpyHostToDevice, st));
+  CU(sci_launch_chirp_tables(e0 * ctx->dt, de * ctx->dt, cv.rows, k, cblocks, cbsz, pc, hrow, st));
+  CU(sci_launch_chirp_fft(1, hrow, SCI_CHIRP_L, SCI_CHIRP_L, 1, nullptr, nullptr, k, cv.kp, nullptr, HpT, cblocks, cbsz, nullptr, 1, st));
+
+  PropParams P;
+  fill_prop_params(ctx, P, nullptr);
+  P.p0q0 = p0q0;
+  P.stride = ntraj;
+  P.nsteps = ctx->nsteps;
+  P.raw = raw;
+  P.raw_stride = cv.nbatch;
+  P.pq_steps = pqs;
+  P.raw_plain = 1;
+
+  long long tile0 = 0;
+  for (long long j0 = 0; j0 < ntraj; j0 += nbatch) {
+    const long long nb = (ntraj - j0 < nbatch) ? ntraj - j0 : nbatch;
+    P.j0 = j0;
+    P.nb = nb;
+    P.good = good + j0;
+    CU(launch_kernel_a(ctx, P, st));
+    CU(sci_launch_weights(weights ? weights + j0 : nullptr, good + j0, nb, wg + j0, st));
+    const int grid = nb < ctx->sm_count ? (int)nb : ctx->sm_count;
+    for (int n = 0; n < nchi; n++) {
+      CU(sci_launch_zassemble_combo(raw, pqs, cv.nbatch, nb, ctx->nsteps, F, chis_dev, eps_dev + (size_t)n * ncs * 2, ncs, pc, x,
+                                    cv.xstride, st));
+      CU(sci_launch_chirp_fft(0, x, cv.xstride, cv.rows, nb, HpT, wg + j0, k, cv.kp,
+                              partial + ((size_t)n * cv.tiles_per_chi + tile0) * cv.kp, nullptr, cblocks, cbsz, yscr, grid, st));
+    }
+    tile0 += grid;
+  }
+  CU(sci_launch_count_good(good, ntraj, ngood, 0, st));
+  const double T = (double)ctx->nsteps * ctx->dt;
+  const double norm = ctx->dt * ctx->dt / (pow(2.0 * M_PI, F + 1) * T);
+  for (int n = 0; n < nchi; n++)
+    CU(sci_launch_final(partial + (size_t)n * cv.tiles_per_chi * cv.kp, tile0, cv.kp, k, ngood, norm, I_out + (size_t)n * k, st));
+  long long ng = 0;
+  CU(cudaMemcpyAsync(&ng, ngood, sizeof(long long), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  if (n_good_out) *n_good_out = ng;
+  if (ng == 0) return fail(ctx, SC_IVR_ENOGOOD, "every trajectory was rejected");
+  return SC_IVR_OK;
+}
+
+}  // extern "C"

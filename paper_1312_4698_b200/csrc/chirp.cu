@@ -399,6 +399,72 @@ __global__ void __maxnreg__(SCI_ZREG) k_zassemble_rows(const double4 *__restrict
   }
 }
 
+// z assembly for a reference state that is a combination of coherent states (row f4):
+//   <chi|p q> = sum_m conj(eps_m) exp(a_m + i b_m),  a_m, b_m of Eq. 3 for |p_m, q_m>   (reduced coordinates)
+//   x_c = <chi|p q> e^{i S} u pc[c]
+// from the plain records (0, S, Re D, Im D) and the (P, Q) of every step.  Same tiling as k_zassemble_rows.
+__global__ void __maxnreg__(128) k_zassemble_combo(const double4 *__restrict__ raw, const double2 *__restrict__ pqs, long long raw_stride,
+                                                   long long nb, int nsteps, int F, const double *__restrict__ chis,
+                                                   const double *__restrict__ eps, int ncs, const double2 *__restrict__ pc,
+                                                   double2 *__restrict__ xrows, long long xstride) {
+  __shared__ double2 tile[2][32][33];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long j0 = ((long long)blockIdx.x * 2 + warp) * 32;
+  if (j0 >= nb) return;
+  const long long j = j0 + lane;
+  const long long jr = (j < nb) ? j : nb - 1;
+  double upr = 1.0, upi = 0.0;
+  const int n1 = nsteps + 1;
+  for (int c0 = 0; c0 < n1; c0 += 32) {
+    const int cn = min(32, n1 - c0);
+    for (int cc = 0; cc < cn; cc++) {
+      const int c = c0 + cc;
+      const double4 r = raw[(long long)c * raw_stride + jr];
+      const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
+      const double x = r.z * inv, y = r.w * inv;
+      double ur, ui;
+      if (x >= 0.0) {
+        ur = sqrt(0.5 * (1.0 + x));
+        ui = 0.5 * y / ur;
+      } else {
+        ui = copysign(sqrt(0.5 * (1.0 - x)), y);
+        ur = 0.5 * y / ui;
+      }
+      if (ur * upr + ui * upi < 0.0) {
+        ur = -ur;
+        ui = -ui;
+      }
+      upr = ur;
+      upi = ui;
+      double wr = 0.0, wi = 0.0;  // <chi|p q>
+      for (int m = 0; m < ncs; m++) {
+        double am = 0.0, bm = 0.0;
+        for (int a = 0; a < F; a++) {
+          const double2 pq = pqs[((long long)c * F + a) * raw_stride + jr];
+          const double dq = chis[(2 * m + 1) * F + a] - pq.y, dp = chis[2 * m * F + a] - pq.x;
+          am = fma(-0.25, fma(dq, dq, dp * dp), am);
+          bm = fma(0.5 * (chis[2 * m * F + a] + pq.x), dq, bm);
+        }
+        const double ea = exp(am);
+        double s, co;
+        sincos(bm, &s, &co);
+        const double er = eps[2 * m], ei = -eps[2 * m + 1];  // conj(eps_m)
+        wr = fma(ea, er * co - ei * s, wr);
+        wi = fma(ea, er * s + ei * co, wi);
+      }
+      double s, co;
+      sincos(r.y, &s, &co);
+      const double2 ph = make_double2(co * ur - s * ui, co * ui + s * ur);  // e^{iS} u
+      tile[warp][lane][cc] = cmul(cmul(make_double2(wr, wi), ph), pc[c]);
+    }
+    __syncwarp();
+    for (int rr = 0; rr < 32; rr++) {
+      if (j0 + rr < nb && lane < cn) xrows[(j0 + rr) * xstride + c0 + lane] = tile[warp][rr][lane];
+    }
+    __syncwarp();
+  }
+}
+
 // parity entry only: x[j][c] = z[c][j] pc[c] from a time-major z series
 __global__ void k_rows_from_z(const double2 *__restrict__ z, long long n, int n1, const double2 *__restrict__ pc,
                               double2 *__restrict__ xrows, long long xstride) {
@@ -458,5 +524,14 @@ cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const 
                                    cudaStream_t st) {
   const long long tot = n * n1;
   k_rows_from_z<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(z, n, n1, pc, xrows, xstride);
+  return cudaGetLastError();
+}
+
+cudaError_t sci_launch_zassemble_combo(const double4 *raw, const double2 *pq_steps, long long raw_stride, long long nb, int nsteps, int F,
+                                       const double *chis_reduced, const double *eps, int ncs, const double2 *pc, double2 *xrows,
+                                       long long xstride, cudaStream_t st) {
+  const long long warps = (nb + 31) / 32;
+  k_zassemble_combo<<<(unsigned)((warps + 1) / 2), 64, 0, st>>>(raw, pq_steps, raw_stride, nb, nsteps, F, chis_reduced, eps, ncs, pc,
+                                                                 xrows, xstride);
   return cudaGetLastError();
 }

@@ -34,6 +34,11 @@ struct PropParams {
   const double *coef;            // packed reduced PES coefficients (device)
   double4 *raw;                  // [nsteps+1][raw_stride]: (ln|<chi|pq>|, S + arg<chi|pq>, Re det 2K, Im det 2K); may be NULL
   long long raw_stride;
+  // several reference states per run (row f4): when pq_steps != NULL the kernel also stores (P_a, Q_a) (reduced) of every
+  // step, [nsteps+1][F][raw_stride], and with raw_plain != 0 the record is (0, S, Re det 2K, Im det 2K): the overlaps are
+  // then formed per reference state by the z assembly
+  double2 *pq_steps;
+  int raw_plain;
   unsigned char *good;           // [nb]; may be NULL
   // debug outputs (may be NULL), indexed by the GLOBAL trajectory number j0 + jj with stride `stride`
   double *pq_out, *S_out, *M_out;
@@ -109,6 +114,9 @@ cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, in
                                     cudaStream_t st);
 cudaError_t sci_launch_zassemble_rows(const double4 *raw, long long raw_stride, long long nb, int nsteps, const double2 *pc,
                                       double2 *xrows, long long xstride, cudaStream_t st);
+cudaError_t sci_launch_zassemble_combo(const double4 *raw, const double2 *pq_steps, long long raw_stride, long long nb, int nsteps, int F,
+                                       const double *chis_reduced /*[ncs][2F]: P_eq then Q_eq*/, const double *eps /*[ncs][2]*/, int ncs,
+                                       const double2 *pc, double2 *xrows, long long xstride, cudaStream_t st);
 cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const double2 *pc, double2 *xrows, long long xstride,
                                    cudaStream_t st);
 cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, int n1, long long nrows, const double2 *HpT,

@@ -470,6 +470,11 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
       const double dq = Qeq_a - Q, dp = Peq_a - Pm;
       oa = -0.25 * fma(dq, dq, dp * dp);
       ob = fma(0.5 * (Peq_a + Pm), dq, Sa);
+      if (P.raw_plain) {  // several reference states: the record carries S alone, (P, Q) of the step go out beside it
+        oa = 0.0;
+        ob = Sa;
+      }
+      if (P.pq_steps != nullptr && valid) P.pq_steps[((long long)c * F + a) * P.raw_stride + jj] = make_double2(Pm, Q);
       if (F > 1) red[a] = make_double2(oa, ob);
     }
     // working copies for the two eliminations: column a of 2K (a5; Eq. 5, R2) and columns a, F+a of M (a7)

@@ -258,6 +258,11 @@ __global__ void __launch_bounds__(kTptThreads) k_propagate_tpt(const __grid_cons
       const double dq = P.Qeq[a] - Q[a], dp = P.Peq[a] - Pm[a];
       oa = fma(-0.25, fma(dq, dq, dp * dp), oa);
       ob = fma(0.5 * (P.Peq[a] + Pm[a]), dq, ob);
+      if (P.pq_steps != nullptr && valid) P.pq_steps[((long long)cstep * F + a) * P.raw_stride + jj] = make_double2(Pm[a], Q[a]);
+    }
+    if (P.raw_plain) {  // several reference states: the record carries S alone
+      oa = 0.0;
+      ob = S;
     }
     // a5: det 2K (Eq. 5, R2)
     double Dre, Dim;

@@ -206,6 +206,51 @@ def test_run_long_series_takes_the_blocked_chirp_path(torch_cuda, B, oracle):
     _assert_spectrum(oracle, I.cpu().numpy(), Io)
 
 
+@pytest.mark.parametrize("cfg,ntraj,nsteps", [(2, 150, 900), (4, 77, 500), (1, 64, 700)])
+def test_run_multi_reference_states(torch_cuda, B, oracle, cfg, ntraj, nsteps):
+    """Row f4: several reference states, each a combination of coherent states, from ONE propagation.
+    Every I_n must match the oracle's run with that combination; the plain state (1, 0, 0) must equal sc_ivr_run."""
+    torch = torch_cuda
+    w = inputs.make_config(cfg, ntraj=ntraj, nsteps=nsteps, k=257)
+    F = w.F
+    rng = np.random.default_rng(17)
+    flip = np.concatenate([-np.ones(F), np.ones(F)])                   # p -> -p
+    chis = np.stack([w.chi, w.chi * flip, w.chi + 0.05 * np.abs(w.chi).max() * rng.standard_normal(2 * F)])
+    eps = np.array([[1.0, 0.0, 0.0], [1.0, 1.0, 0.0], [1.0, -1.0, 0.0], [0.5, 0.25j, -0.75 + 0.1j]])
+    ctx = B.ScIvr.from_workload(w)
+    dev = _dev(torch, w.p0q0)
+    I, ng, rc = ctx.run_multi(dev, chis, eps, w.E)
+    I = I.cpu().numpy()
+    for n in range(eps.shape[0]):
+        Io, ngo, rco = oracle.run_combo(F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, chis, eps[n], w.E)
+        assert (ng, rc) == (ngo, rco)
+        assert np.max(np.abs(I[n] - Io)) <= TOL_I * Io.max(), n
+    I1, ng1, rc1 = ctx.run(dev, w.chi, w.E)
+    assert ng1 == ng
+    assert np.max(np.abs(I[0] - I1.cpu().numpy())) <= 1e-12 * I[0].max()
+
+
+def test_run_multi_batches_and_errors(torch_cuda, B, oracle):
+    torch = torch_cuda
+    w = inputs.make_config(2, ntraj=3000, nsteps=300, k=64)
+    ctx = B.ScIvr.from_workload(w)
+    dev = _dev(torch, w.p0q0)
+    chis = np.stack([w.chi, -w.chi])
+    eps = np.array([[1.0, 1.0], [1.0, -1.0]])
+    Ia, nga, _ = ctx.run_multi(dev, chis, eps, w.E)
+    small = torch.empty(ctx._lib_multi_bytes(w.ntraj, w.k, ctx.min_batch()), dtype=torch.uint8, device="cuda")
+    Ib, ngb, _ = ctx.run_multi(dev, chis, eps, w.E, workspace=small)   # several batches
+    assert nga == ngb == w.ntraj
+    assert np.max(np.abs((Ia - Ib).cpu().numpy())) <= 1e-12 * Ia.max().item()
+    Io, _, _ = oracle.run_combo(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, chis, eps[1], w.E)
+    assert np.max(np.abs(Ib[1].cpu().numpy() - Io)) <= TOL_I * Io.max()
+    E = w.E.copy()
+    E[3] *= 1.001
+    with pytest.raises(B.ScIvrError) as ei:
+        ctx.run_multi(dev, chis, eps, E)
+    assert ei.value.status == 4
+
+
 def _run_both(torch, B, oracle, w, **kw):
     ctx = B.ScIvr.from_workload(w, **kw)
     I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
