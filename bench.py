@@ -148,6 +148,8 @@ def main():
     ap.add_argument("--det-stride", type=int, default=1)
     ap.add_argument("--ref-sample", type=int, default=1024)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nchi", type=int, default=0,
+                    help="measure sc_ivr_run_multi with this many reference states (row f4) instead of sc_ivr_run; short JSON line")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -184,6 +186,27 @@ def main():
 
     def step():
         ctx.run(d_pq, w.chi, w.E, I_out=I_dev, workspace=wsp, want_n_good=False)
+
+    if args.nchi > 0:  # row f4: nchi combinations of the states (+-p_eq, q_eq) sharing one propagation
+        del wsp
+        F = w.F
+        chis = np.stack([w.chi, w.chi * np.concatenate([-np.ones(F), np.ones(F)])])
+        eps = np.array([[1.0, np.cos(np.pi * n / max(1, args.nchi - 1))] for n in range(args.nchi)])
+        wsm = torch.empty(ctx._lib_multi_bytes(w.ntraj, w.k), dtype=torch.uint8, device="cuda")
+        for _ in range(args.warmup):
+            ctx.run_multi(d_pq, chis, eps, w.E, workspace=wsm)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            ctx.run_multi(d_pq, chis, eps, w.E, workspace=wsm)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        print(json.dumps({"metric": METRIC + ", shared by nchi reference states", "value": w.ntraj * w.nsteps / (ms * 1e-3), "unit": UNIT,
+                          "nchi": args.nchi, "ms_per_step": ms, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+                          "config": {"workload": w.name, "F": w.F, "ntraj_per_gpu": w.ntraj, "nsteps": w.nsteps, "k": w.k}}))
+        return
 
     for _ in range(args.warmup):
         step()
