@@ -701,7 +701,8 @@ int occupancy() {
 
 }  // namespace
 
-#define SCI_FOR_EACH_F(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
+// F <= SCI_TPT_MAXF is served by the thread-per-trajectory kernels (propagate_tpt.cu)
+#define SCI_FOR_EACH_F(X) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12)
 
 int sci_prop_traj_per_block(int F) { return (kThreads / 32) * (32 / F); }
 
