@@ -192,7 +192,7 @@ def main():
         F = w.F
         chis = np.stack([w.chi, w.chi * np.concatenate([-np.ones(F), np.ones(F)])])
         eps = np.array([[1.0, np.cos(np.pi * n / max(1, args.nchi - 1))] for n in range(args.nchi)])
-        wsm = torch.empty(ctx._lib_multi_bytes(w.ntraj, w.k), dtype=torch.uint8, device="cuda")
+        wsm = torch.empty(ctx._lib_multi_bytes(w.ntraj, w.k, 2), dtype=torch.uint8, device="cuda")
         for _ in range(args.warmup):
             ctx.run_multi(d_pq, chis, eps, w.E, workspace=wsm)
         torch.cuda.synchronize()

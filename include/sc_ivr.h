@@ -142,12 +142,12 @@ sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double 
  * Fourier / reduction stages (a8, a9) are repeated per state.
  *   chis  HOST [ncs][2F]  (p_m[F] then q_m[F])        eps  HOST [nchi][ncs][2]  (re, im)
  *   I_out DEVICE [nchi][k]                             E    HOST [k], equally spaced (chirp-z path only)
- *   workspace DEVICE, sc_ivr_multi_workspace_bytes(ctx, ntraj, k, max_batch); a smaller one (>= one batch of
+ *   workspace DEVICE, sc_ivr_multi_workspace_bytes(ctx, ntraj, k, ncs, max_batch); a smaller one (>= one batch of
  *   sc_ivr_min_batch) makes more, smaller batches.  1 <= ncs <= 16, 1 <= nchi <= 16.
  * Other arguments, ordering and error behaviour as sc_ivr_run; SC_IVR_EUNSUPPORTED when the grid is not equally spaced or too
  * long for the chirp-z stage.
  */
-size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, long long max_batch /*0 = 32768*/);
+size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, int ncs, long long max_batch /*0 = 32768*/);
 sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chis,
                                int ncs, const double *eps, int nchi, const double *E, int k, double *I_out,
                                long long *n_good_out, void *workspace, size_t workspace_bytes, void *cuda_stream);

@@ -78,7 +78,7 @@ def lib():
     L.sc_ivr_fourier_workspace_bytes.restype = C.c_size_t
     L.sc_ivr_fourier_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int]
     L.sc_ivr_multi_workspace_bytes.restype = C.c_size_t
-    L.sc_ivr_multi_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int, C.c_longlong]
+    L.sc_ivr_multi_workspace_bytes.argtypes = [_vp, C.c_longlong, C.c_int, C.c_int, C.c_longlong]
     L.sc_ivr_run_multi.restype = C.c_int
     L.sc_ivr_run_multi.argtypes = [_vp, _vp, _vp, C.c_longlong, _dp, C.c_int, _dp, C.c_int, _dp, C.c_int, _vp,
                                    C.POINTER(C.c_longlong), _vp, C.c_size_t, _vp]
@@ -254,8 +254,8 @@ class ScIvr:
         self._check(lib().sc_ivr_eval_pes(self._h, _dev(q), n, _dev(V), _dev(g), _dev(H), _stream()))
         return V, g, H
 
-    def _lib_multi_bytes(self, ntraj, k, max_batch=0):
-        return int(lib().sc_ivr_multi_workspace_bytes(self._h, int(ntraj), int(k), int(max_batch)))
+    def _lib_multi_bytes(self, ntraj, k, ncs, max_batch=0):
+        return int(lib().sc_ivr_multi_workspace_bytes(self._h, int(ntraj), int(k), int(ncs), int(max_batch)))
 
     def run_multi(self, p0q0, chis, eps, E, weights=None, workspace=None, max_batch=0):
         """sc_ivr_run_multi: reference states |chi_n> = sum_m eps[n][m] |chis[m]>; p0q0 DEVICE [2F, ntraj];
@@ -271,7 +271,7 @@ class ScIvr:
         E = _host(E)
         I = torch.empty((nchi, E.size), dtype=torch.float64, device=p0q0.device)
         if workspace is None:
-            workspace = _workspace(lib().sc_ivr_multi_workspace_bytes(self._h, ntraj, E.size, int(max_batch)), p0q0.device)
+            workspace = _workspace(self._lib_multi_bytes(ntraj, E.size, ncs, max_batch), p0q0.device)
         ng = C.c_longlong(0)
         rc = lib().sc_ivr_run_multi(self._h, _dev(p0q0), _dev(weights) if weights is not None else None, ntraj, _hp(chis), ncs,
                                     _hp(ee), nchi, _hp(E), E.size, _dev(I), C.byref(ng), _dev(workspace), workspace.numel(),

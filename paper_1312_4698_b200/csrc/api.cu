@@ -612,9 +612,9 @@ struct CarveMulti {
   long long nbatch, xstride;
   int rows, kp;
   long long tiles_per_chi;  // partial rows per reference state
-  size_t off_raw, off_pq, off_x, off_partial, off_good, off_wg, off_ngood, off_pc, off_hrow, off_HpT, off_yscr, off_chis, off_eps, total;
+  size_t off_raw, off_pq, off_ov, off_x, off_partial, off_good, off_wg, off_ngood, off_pc, off_hrow, off_HpT, off_yscr, off_chis, off_eps, total;
 };
-CarveMulti carve_multi(const sc_ivr_ctx *ctx, long long ntraj, int k, long long nbatch) {
+CarveMulti carve_multi(const sc_ivr_ctx *ctx, long long ntraj, int k, int ncs, long long nbatch) {
   CarveMulti c;
   c.nbatch = nbatch;
   c.rows = ctx->nsteps + 1;
@@ -625,6 +625,7 @@ CarveMulti carve_multi(const sc_ivr_ctx *ctx, long long ntraj, int k, long long 
   size_t o = 0;
   c.off_raw = o; o = align_up(o + sizeof(double4) * (size_t)c.rows * (size_t)nbatch, 256);
   c.off_pq = o; o = align_up(o + sizeof(double2) * (size_t)c.rows * (size_t)ctx->F * (size_t)nbatch, 256);
+  c.off_ov = o; o = align_up(o + sizeof(double2) * (size_t)c.rows * (size_t)(ncs + 1) * (size_t)nbatch, 256);
   c.off_x = o; o = align_up(o + sizeof(double2) * (size_t)c.xstride * (size_t)nbatch, 256);
   c.off_partial = o; o = align_up(o + sizeof(double) * 16 * (size_t)c.tiles_per_chi * (size_t)c.kp, 256);
   c.off_good = o; o = align_up(o + (size_t)ntraj, 256);
@@ -643,9 +644,9 @@ CarveMulti carve_multi(const sc_ivr_ctx *ctx, long long ntraj, int k, long long 
 
 extern "C" {
 
-size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, long long max_batch) {
-  if (!ctx || ntraj < 1 || k < 1) return 0;
-  return carve_multi(ctx, ntraj, k, default_batch(ctx, ntraj, max_batch > 0 ? max_batch : 32768)).total;
+size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, int ncs, long long max_batch) {
+  if (!ctx || ntraj < 1 || k < 1 || ncs < 1 || ncs > 16) return 0;
+  return carve_multi(ctx, ntraj, k, ncs, default_batch(ctx, ntraj, max_batch > 0 ? max_batch : 32768)).total;
 }
 
 sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chis,
@@ -668,18 +669,19 @@ sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double
   cudaStream_t st = (cudaStream_t)cuda_stream;
 
   long long nbatch = default_batch(ctx, ntraj, 32768);
-  CarveMulti cv = carve_multi(ctx, ntraj, k, nbatch);
+  CarveMulti cv = carve_multi(ctx, ntraj, k, ncs, nbatch);
   while (cv.total > workspace_bytes && nbatch > ctx->wave) {
     long long nx = nbatch / 2 / ctx->wave * ctx->wave;
     if (nx < ctx->wave) nx = ctx->wave;
     nbatch = nx;
-    cv = carve_multi(ctx, ntraj, k, nbatch);
+    cv = carve_multi(ctx, ntraj, k, ncs, nbatch);
   }
   if (cv.total > workspace_bytes)
     return fail(ctx, SC_IVR_EINVAL, "workspace too small: %zu bytes given, %zu needed for the minimum batch of %lld", workspace_bytes,
                 cv.total, nbatch);
   char *ws = (char *)workspace;
   double4 *raw = (double4 *)(ws + cv.off_raw);
+  double2 *ovph = (double2 *)(ws + cv.off_ov);
   double2 *pqs = (double2 *)(ws + cv.off_pq);
   double2 *x = (double2 *)(ws + cv.off_x);
   double *partial = (double *)(ws + cv.off_partial);
@@ -726,9 +728,9 @@ sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double
     CU(launch_kernel_a(ctx, P, st));
     CU(sci_launch_weights(weights ? weights + j0 : nullptr, good + j0, nb, wg + j0, st));
     const int grid = nb < ctx->sm_count ? (int)nb : ctx->sm_count;
+    CU(sci_launch_overlap_phase(raw, pqs, cv.nbatch, nb, ctx->nsteps, F, chis_dev, ncs, pc, ovph, st));
     for (int n = 0; n < nchi; n++) {
-      CU(sci_launch_zassemble_combo(raw, pqs, cv.nbatch, nb, ctx->nsteps, F, chis_dev, eps_dev + (size_t)n * ncs * 2, ncs, pc, x,
-                                    cv.xstride, st));
+      CU(sci_launch_combine_rows(ovph, cv.nbatch, nb, ctx->nsteps, eps_dev + (size_t)n * ncs * 2, ncs, x, cv.xstride, st));
       CU(sci_launch_chirp_fft(0, x, cv.xstride, cv.rows, nb, HpT, wg + j0, k, cv.kp,
                               partial + ((size_t)n * cv.tiles_per_chi + tile0) * cv.kp, nullptr, cblocks, cbsz, yscr, grid, st));
     }

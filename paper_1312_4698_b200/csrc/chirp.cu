@@ -399,70 +399,80 @@ __global__ void __maxnreg__(SCI_ZREG) k_zassemble_rows(const double4 *__restrict
   }
 }
 
-// z assembly for a reference state that is a combination of coherent states (row f4):
-//   <chi|p q> = sum_m conj(eps_m) exp(a_m + i b_m),  a_m, b_m of Eq. 3 for |p_m, q_m>   (reduced coordinates)
-//   x_c = <chi|p q> e^{i S} u pc[c]
-// from the plain records (0, S, Re D, Im D) and the (P, Q) of every step.  Same tiling as k_zassemble_rows.
-__global__ void __maxnreg__(128) k_zassemble_combo(const double4 *__restrict__ raw, const double2 *__restrict__ pqs, long long raw_stride,
-                                                   long long nb, int nsteps, int F, const double *__restrict__ chis,
-                                                   const double *__restrict__ eps, int ncs, const double2 *__restrict__ pc,
-                                                   double2 *__restrict__ xrows, long long xstride) {
+// z assembly for reference states that are combinations of coherent states (row f4), in two stages so
+// that the (P, Q) stream is read once per batch, not once per reference state:
+//   stage 1 (k_overlap_phase, one thread per trajectory, sequential in c for the branch rule R6):
+//       ph[c][j]    = e^{i S} u pc[c]                       from the plain records (0, S, Re D, Im D)
+//       ov[c][m][j] = exp(a_m + i b_m) = <p_m q_m|p q>      (Eq. 3, reduced coordinates) for every coherent state m
+//   stage 2 (k_combine_rows, per reference state n, fully parallel):
+//       x_n[j][c]   = ph[c][j] * sum_m conj(eps_nm) ov[c][m][j],   transposed to trajectory-major rows for the chirp-z stage
+__global__ void __maxnreg__(128) k_overlap_phase(const double4 *__restrict__ raw, const double2 *__restrict__ pqs, long long raw_stride,
+                                                 long long nb, int nsteps, int F, const double *__restrict__ chis, int ncs,
+                                                 const double2 *__restrict__ pc, double2 *__restrict__ ovph) {
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= nb) return;
+  double upr = 1.0, upi = 0.0;
+  for (int c = 0; c <= nsteps; c++) {
+    const double4 r = raw[(long long)c * raw_stride + j];
+    const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
+    const double x = r.z * inv, y = r.w * inv;
+    double ur, ui;
+    if (x >= 0.0) {
+      ur = sqrt(0.5 * (1.0 + x));
+      ui = 0.5 * y / ur;
+    } else {
+      ui = copysign(sqrt(0.5 * (1.0 - x)), y);
+      ur = 0.5 * y / ui;
+    }
+    if (ur * upr + ui * upi < 0.0) {
+      ur = -ur;
+      ui = -ui;
+    }
+    upr = ur;
+    upi = ui;
+    double s, co;
+    sincos(r.y, &s, &co);
+    double2 *o = ovph + (long long)c * (ncs + 1) * raw_stride + j;
+    o[0] = cmul(make_double2(co * ur - s * ui, co * ui + s * ur), pc[c]);
+    for (int m = 0; m < ncs; m++) {
+      double am = 0.0, bm = 0.0;
+      for (int a = 0; a < F; a++) {
+        const double2 pq = pqs[((long long)c * F + a) * raw_stride + j];
+        const double dq = chis[(2 * m + 1) * F + a] - pq.y, dp = chis[2 * m * F + a] - pq.x;
+        am = fma(-0.25, fma(dq, dq, dp * dp), am);
+        bm = fma(0.5 * (chis[2 * m * F + a] + pq.x), dq, bm);
+      }
+      const double ea = exp(am);
+      sincos(bm, &s, &co);
+      o[(long long)(m + 1) * raw_stride] = make_double2(ea * co, ea * s);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(64) k_combine_rows(const double2 *__restrict__ ovph, long long raw_stride, long long nb, int nsteps,
+                                                     const double *__restrict__ eps, int ncs, double2 *__restrict__ xrows,
+                                                     long long xstride) {
   __shared__ double2 tile[2][32][33];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long j0 = ((long long)blockIdx.x * 2 + warp) * 32;
+  const int c0 = blockIdx.y * 32;
   if (j0 >= nb) return;
-  const long long j = j0 + lane;
-  const long long jr = (j < nb) ? j : nb - 1;
-  double upr = 1.0, upi = 0.0;
-  const int n1 = nsteps + 1;
-  for (int c0 = 0; c0 < n1; c0 += 32) {
-    const int cn = min(32, n1 - c0);
-    for (int cc = 0; cc < cn; cc++) {
-      const int c = c0 + cc;
-      const double4 r = raw[(long long)c * raw_stride + jr];
-      const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
-      const double x = r.z * inv, y = r.w * inv;
-      double ur, ui;
-      if (x >= 0.0) {
-        ur = sqrt(0.5 * (1.0 + x));
-        ui = 0.5 * y / ur;
-      } else {
-        ui = copysign(sqrt(0.5 * (1.0 - x)), y);
-        ur = 0.5 * y / ui;
-      }
-      if (ur * upr + ui * upi < 0.0) {
-        ur = -ur;
-        ui = -ui;
-      }
-      upr = ur;
-      upi = ui;
-      double wr = 0.0, wi = 0.0;  // <chi|p q>
-      for (int m = 0; m < ncs; m++) {
-        double am = 0.0, bm = 0.0;
-        for (int a = 0; a < F; a++) {
-          const double2 pq = pqs[((long long)c * F + a) * raw_stride + jr];
-          const double dq = chis[(2 * m + 1) * F + a] - pq.y, dp = chis[2 * m * F + a] - pq.x;
-          am = fma(-0.25, fma(dq, dq, dp * dp), am);
-          bm = fma(0.5 * (chis[2 * m * F + a] + pq.x), dq, bm);
-        }
-        const double ea = exp(am);
-        double s, co;
-        sincos(bm, &s, &co);
-        const double er = eps[2 * m], ei = -eps[2 * m + 1];  // conj(eps_m)
-        wr = fma(ea, er * co - ei * s, wr);
-        wi = fma(ea, er * s + ei * co, wi);
-      }
-      double s, co;
-      sincos(r.y, &s, &co);
-      const double2 ph = make_double2(co * ur - s * ui, co * ui + s * ur);  // e^{iS} u
-      tile[warp][lane][cc] = cmul(cmul(make_double2(wr, wi), ph), pc[c]);
+  const long long j = (j0 + lane < nb) ? j0 + lane : nb - 1;
+  const int cn = min(32, nsteps + 1 - c0);
+  for (int cc = 0; cc < cn; cc++) {
+    const double2 *o = ovph + (long long)(c0 + cc) * (ncs + 1) * raw_stride + j;
+    double wr = 0.0, wi = 0.0;
+    for (int m = 0; m < ncs; m++) {
+      const double2 v = o[(long long)(m + 1) * raw_stride];
+      const double er = eps[2 * m], ei = -eps[2 * m + 1];  // conj(eps_m)
+      wr += er * v.x - ei * v.y;
+      wi += er * v.y + ei * v.x;
     }
-    __syncwarp();
-    for (int rr = 0; rr < 32; rr++) {
-      if (j0 + rr < nb && lane < cn) xrows[(j0 + rr) * xstride + c0 + lane] = tile[warp][rr][lane];
-    }
-    __syncwarp();
+    tile[warp][lane][cc] = cmul(make_double2(wr, wi), o[0]);
   }
+  __syncwarp();
+  for (int rr = 0; rr < 32; rr++)
+    if (j0 + rr < nb && lane < cn) xrows[(j0 + rr) * xstride + c0 + lane] = tile[warp][rr][lane];
 }
 
 // parity entry only: x[j][c] = z[c][j] pc[c] from a time-major z series
@@ -527,11 +537,16 @@ cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const 
   return cudaGetLastError();
 }
 
-cudaError_t sci_launch_zassemble_combo(const double4 *raw, const double2 *pq_steps, long long raw_stride, long long nb, int nsteps, int F,
-                                       const double *chis_reduced, const double *eps, int ncs, const double2 *pc, double2 *xrows,
-                                       long long xstride, cudaStream_t st) {
+cudaError_t sci_launch_overlap_phase(const double4 *raw, const double2 *pq_steps, long long raw_stride, long long nb, int nsteps, int F,
+                                     const double *chis_reduced, int ncs, const double2 *pc, double2 *ovph, cudaStream_t st) {
+  k_overlap_phase<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(raw, pq_steps, raw_stride, nb, nsteps, F, chis_reduced, ncs, pc, ovph);
+  return cudaGetLastError();
+}
+
+cudaError_t sci_launch_combine_rows(const double2 *ovph, long long raw_stride, long long nb, int nsteps, const double *eps, int ncs,
+                                    double2 *xrows, long long xstride, cudaStream_t st) {
   const long long warps = (nb + 31) / 32;
-  k_zassemble_combo<<<(unsigned)((warps + 1) / 2), 64, 0, st>>>(raw, pq_steps, raw_stride, nb, nsteps, F, chis_reduced, eps, ncs, pc,
-                                                                 xrows, xstride);
+  dim3 grid((unsigned)((warps + 1) / 2), (unsigned)((nsteps + 1 + 31) / 32));
+  k_combine_rows<<<grid, 64, 0, st>>>(ovph, raw_stride, nb, nsteps, eps, ncs, xrows, xstride);
   return cudaGetLastError();
 }

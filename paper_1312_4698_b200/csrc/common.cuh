@@ -114,9 +114,11 @@ cudaError_t sci_launch_chirp_tables(double e0dt, double theta, int n1, int k, in
                                     cudaStream_t st);
 cudaError_t sci_launch_zassemble_rows(const double4 *raw, long long raw_stride, long long nb, int nsteps, const double2 *pc,
                                       double2 *xrows, long long xstride, cudaStream_t st);
-cudaError_t sci_launch_zassemble_combo(const double4 *raw, const double2 *pq_steps, long long raw_stride, long long nb, int nsteps, int F,
-                                       const double *chis_reduced /*[ncs][2F]: P_eq then Q_eq*/, const double *eps /*[ncs][2]*/, int ncs,
-                                       const double2 *pc, double2 *xrows, long long xstride, cudaStream_t st);
+cudaError_t sci_launch_overlap_phase(const double4 *raw, const double2 *pq_steps, long long raw_stride, long long nb, int nsteps, int F,
+                                     const double *chis_reduced /*[ncs][2F]: P_eq then Q_eq*/, int ncs, const double2 *pc,
+                                     double2 *ovph /*[nsteps+1][ncs+1][raw_stride]*/, cudaStream_t st);
+cudaError_t sci_launch_combine_rows(const double2 *ovph, long long raw_stride, long long nb, int nsteps, const double *eps /*[ncs][2]*/,
+                                    int ncs, double2 *xrows, long long xstride, cudaStream_t st);
 cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const double2 *pc, double2 *xrows, long long xstride,
                                    cudaStream_t st);
 cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, int n1, long long nrows, const double2 *HpT,

@@ -238,7 +238,7 @@ def test_run_multi_batches_and_errors(torch_cuda, B, oracle):
     chis = np.stack([w.chi, -w.chi])
     eps = np.array([[1.0, 1.0], [1.0, -1.0]])
     Ia, nga, _ = ctx.run_multi(dev, chis, eps, w.E)
-    small = torch.empty(ctx._lib_multi_bytes(w.ntraj, w.k, ctx.min_batch()), dtype=torch.uint8, device="cuda")
+    small = torch.empty(ctx._lib_multi_bytes(w.ntraj, w.k, 2, ctx.min_batch()), dtype=torch.uint8, device="cuda")
     Ib, ngb, _ = ctx.run_multi(dev, chis, eps, w.E, workspace=small)   # several batches
     assert nga == ngb == w.ntraj
     assert np.max(np.abs((Ia - Ib).cpu().numpy())) <= 1e-12 * Ia.max().item()
