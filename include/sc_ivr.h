@@ -203,6 +203,10 @@ sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *z, long long n
  * last event.  Timing is recorded only after sc_ivr_set_timing(ctx, 1).
  */
 sc_ivr_status sc_ivr_fp64_probe(int mode, int iters, double *flops_out, double *ms_out);
+/* Number of trajectory-steps of the most recent sc_ivr_run with n_good_out != NULL (or sc_ivr_run_host) on ctx whose
+ * determinants were repeated with the pivoted eliminations because a multiplier of the fixed-order elimination exceeded
+ * lu_growth_max; -1 when that run did not read it back.  Statistics only. */
+long long sc_ivr_last_fallbacks(const sc_ivr_ctx *ctx);
 void sc_ivr_set_timing(sc_ivr_ctx *ctx, int on);
 sc_ivr_status sc_ivr_last_timings(sc_ivr_ctx *ctx, double out[6]);
 

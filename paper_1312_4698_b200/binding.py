@@ -22,7 +22,7 @@ EXPORTS = [
     "sc_ivr_run", "sc_ivr_host_staging_bytes", "sc_ivr_run_host", "sc_ivr_propagate_workspace_bytes",
     "sc_ivr_propagate", "sc_ivr_eval_pes", "sc_ivr_fourier_workspace_bytes", "sc_ivr_fourier",
     "sc_ivr_fourier_power_workspace_bytes", "sc_ivr_fourier_power", "sc_ivr_multi_workspace_bytes", "sc_ivr_run_multi",
-    "sc_ivr_fp64_probe", "sc_ivr_set_timing", "sc_ivr_last_timings",
+    "sc_ivr_fp64_probe", "sc_ivr_set_timing", "sc_ivr_last_timings", "sc_ivr_last_fallbacks",
 ]
 
 
@@ -169,6 +169,12 @@ class ScIvr:
 
     def host_staging_bytes(self, ntraj, k):
         return int(lib().sc_ivr_host_staging_bytes(self._h, int(ntraj), int(k)))
+
+    def last_fallbacks(self):
+        """Trajectory-steps of the last synchronising run that needed the pivoted eliminations (-1: not read back)."""
+        f = lib().sc_ivr_last_fallbacks
+        f.restype, f.argtypes = C.c_longlong, [_vp]
+        return int(f(self._h))
 
     def set_timing(self, on=True):
         lib().sc_ivr_set_timing(self._h, 1 if on else 0)

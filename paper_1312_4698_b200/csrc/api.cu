@@ -413,6 +413,9 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
   P.nsteps = ctx->nsteps;
   P.raw = raw;
   P.raw_stride = cv.nbatch;
+  P.fb_count = (unsigned long long *)(ngood + 1);
+  CU(cudaMemsetAsync(ngood + 1, 0, sizeof(long long), st));
+  ctx->last_fallbacks = -1;
 
   long long tile0 = 0;
   for (long long j0 = 0; j0 < ntraj; j0 += nbatch) {
@@ -454,14 +457,17 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
   ctx->tms[5] = launches;
 
   if (n_good_out) {
-    long long ng = 0;
-    CU(cudaMemcpyAsync(&ng, ngood, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    long long ng[2] = {0, 0};
+    CU(cudaMemcpyAsync(ng, ngood, 2 * sizeof(long long), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
-    *n_good_out = ng;
-    if (ng == 0) return fail(ctx, SC_IVR_ENOGOOD, "every trajectory was rejected");
+    *n_good_out = ng[0];
+    ctx->last_fallbacks = ng[1];
+    if (ng[0] == 0) return fail(ctx, SC_IVR_ENOGOOD, "every trajectory was rejected");
   }
   return SC_IVR_OK;
 }
+
+long long sc_ivr_last_fallbacks(const sc_ivr_ctx *ctx) { return ctx ? ctx->last_fallbacks : -1; }
 
 sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chi,
                               const double *E, int k, double *I_out, long long *n_good_out, void *workspace,

@@ -39,6 +39,7 @@ struct PropParams {
   // then formed per reference state by the z assembly
   double2 *pq_steps;
   int raw_plain;
+  unsigned long long *fb_count;  // may be NULL: number of trajectory-steps repeated with the pivoted eliminations
   unsigned char *good;           // [nb]; may be NULL
   // debug outputs (may be NULL), indexed by the GLOBAL trajectory number j0 + jj with stride `stride`
   double *pq_out, *S_out, *M_out;
@@ -67,6 +68,7 @@ struct sc_ivr_ctx {
   char err[512];
   int timing;
   double tms[6];
+  long long last_fallbacks;  // of the most recent synchronising sc_ivr_run; -1 = not read back
   // stage timing: (start, stop) event pairs recorded without synchronising, resolved by sc_ivr_last_timings
   std::vector<cudaEvent_t> ev;
   std::vector<int> ev_slot;

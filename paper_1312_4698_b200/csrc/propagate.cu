@@ -520,6 +520,7 @@ __global__ void __launch_bounds__(kThreads) k_propagate(const __grid_constant__ 
           Dre = fDre;
           Dim = fDim;
           dM = fdM;
+          if (P.fb_count != nullptr && a == 0 && valid) atomicAdd(P.fb_count, 1ULL);  // statistics only
         }
       }
     }

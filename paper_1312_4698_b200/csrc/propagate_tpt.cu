@@ -290,6 +290,7 @@ __global__ void __launch_bounds__(kTptThreads) k_propagate_tpt(const __grid_cons
       det_pivoted_complex<F>(br, bi, o);
       Dre = o[0];
       Dim = o[1];
+      if (P.fb_count != nullptr && valid) atomicAdd(P.fb_count, 1ULL);  // statistics only
     }
     if (valid && P.raw != nullptr) P.raw[(long long)cstep * P.raw_stride + jj] = make_double4(oa, ob, Dre, Dim);
     // a7: |det M - 1| <= tol and finite
@@ -318,6 +319,7 @@ __global__ void __launch_bounds__(kTptThreads) k_propagate_tpt(const __grid_cons
             buf[(F + i) * 2 * F + F + b] = Mqq[i][b];
           }
         dM = det_pivoted_real<2 * F>(buf);
+        if (P.fb_count != nullptr && valid && growK < P.grow_k_max) atomicAdd(P.fb_count, 1ULL);  // not counted twice
       }
       bool fin = isfinite(S);
 #pragma unroll

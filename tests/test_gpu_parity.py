@@ -251,6 +251,21 @@ def test_run_multi_batches_and_errors(torch_cuda, B, oracle):
     assert ei.value.status == 4
 
 
+@pytest.mark.parametrize("cfg,ntraj", [(2, 96), (4, 60)])
+def test_fallback_statistics(torch_cuda, B, cfg, ntraj):
+    """The fixed-order eliminations are the common path: on the benchmark surfaces the pivoted fallback is (almost) never
+    taken, and with lu_growth_max < 0 it is taken at every trajectory-step."""
+    torch = torch_cuda
+    w = inputs.make_config(cfg, ntraj=ntraj, nsteps=500, k=32)
+    dev = _dev(torch, w.p0q0)
+    ctx = B.ScIvr.from_workload(w)
+    ctx.run(dev, w.chi, w.E)
+    assert 0 <= ctx.last_fallbacks() <= 0.002 * ntraj * 501
+    ctx = B.ScIvr.from_workload(w, lu_growth_max=-1.0)
+    ctx.run(dev, w.chi, w.E)
+    assert ctx.last_fallbacks() == ntraj * 501
+
+
 def _run_both(torch, B, oracle, w, **kw):
     ctx = B.ScIvr.from_workload(w, **kw)
     I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
