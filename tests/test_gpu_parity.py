@@ -266,6 +266,21 @@ def test_fallback_statistics(torch_cuda, B, cfg, ntraj):
     assert ctx.last_fallbacks() == ntraj * 501
 
 
+@pytest.mark.parametrize("F", list(range(1, 13)))
+@pytest.mark.parametrize("integ", [0, 1], ids=["verlet", "fourth_order"])
+def test_run_every_supported_F(torch_cuda, B, oracle, F, integ):
+    """The whole path for every F the library instantiates (thread-per-trajectory kernels F <= 3, F lanes per trajectory
+    above), both integrators, random couplings, ragged sizes: I(E) against the oracle."""
+    torch = torch_cuda
+    w = inputs.make_uncoupled_morse(1, 70, 400, 96, seed=101) if F == 1 else inputs.make_random_qff(F, 40 + 3 * F, 400, 96, seed=101 + F)
+    stride = 1 + 4 * integ
+    ctx = B.ScIvr.from_workload(w, integrator=integ, det_stride=stride)
+    I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
+    Io, ngo, rco = oracle.run_workload(w, integrator=integ, det_stride=stride)
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I.cpu().numpy(), Io)
+
+
 def _run_both(torch, B, oracle, w, **kw):
     ctx = B.ScIvr.from_workload(w, **kw)
     I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
