@@ -14,8 +14,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsc_ivr.so")
-SOURCES = ["api.cu", "propagate.cu", "propagate_tpt.cu", "spectrum.cu", "chirp.cu"]
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(HERE, "..", "include", "sc_ivr.h")]
+SOURCES = ["api.cu", "propagate.cu", "propagate_cml.cu", "propagate_tpt.cu", "spectrum.cu", "chirp.cu"]
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "tmem_ldst.cuh"), os.path.join(HERE, "..", "include", "sc_ivr.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 

@@ -99,6 +99,20 @@ void fill_prop_params(const sc_ivr_ctx *ctx, PropParams &P, const double *chi) {
     P.kick[s] = ctx->sb[s] * ctx->dt;
     P.drift[s] = ctx->sa[s] * ctx->dt;
   }
+  {  // evaluation points: every non-zero drift leaves one; kicks at the step's first point follow the snapshot, the
+     // kicks after the last drift precede the next one
+    int cur = 0, np = 0;
+    for (int s = 0; s < ctx->nstages; s++)
+      if (ctx->sa[s] != 0.0) np++;
+    P.npoints = np;
+    for (int s = 0; s < ctx->nstages; s++) {
+      const double b = ctx->sb[s] * ctx->dt;
+      if (cur == 0) P.pt_post[0] += b;
+      else if (cur == np) P.pt_pre[0] += b;
+      else P.pt_pre[cur] += b;
+      if (ctx->sa[s] != 0.0) P.pt_drift[cur++] = ctx->sa[s] * ctx->dt;
+    }
+  }
   for (int a = 0; a < F; a++) {
     const double sg = sqrt(ctx->gamma[a]);
     P.sg[a] = sg;
@@ -164,6 +178,7 @@ cudaError_t launch_kernel_a(const sc_ivr_ctx *ctx, const PropParams &P, cudaStre
     memcpy(TP.coef, ctx->tpt_coef, sizeof(TP.coef));
     return sci_tpt_launch_propagate(ctx->F, ctx->kind, TP, st);
   }
+  if (sci_cml_lanes(ctx->F)) return sci_cml_launch_propagate(ctx->F, ctx->kind, P, st);
   return sci_launch_propagate(ctx->F, ctx->kind, P, st);
 }
 
@@ -276,9 +291,12 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
       rc = fail(nullptr, SC_IVR_ECUDA, "cannot query the CUDA device");
       break;
     }
-    const size_t nc = sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr);
+    const bool cml = F > SCI_TPT_MAXF && sci_cml_lanes(F) != 0;
+    const size_t nc = cml ? sci_cml_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr)
+                          : sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr);
     std::vector<double> packed(nc + F);  // sqrt(gamma) rides behind the coefficients (for sc_ivr_eval_pes)
-    sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, packed.data());
+    if (cml) sci_cml_pack_coeffs(F, (int)kind, pes_coeffs, gamma, packed.data());
+    else sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, packed.data());
     for (int a = 0; a < F; a++) packed[nc + a] = sqrt(gamma[a]);
     ctx->n_coef = nc;
     if ((ce = cudaMalloc(&ctx->d_coef, sizeof(double) * (nc + F))) != cudaSuccess ||
@@ -290,6 +308,8 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
       memset(ctx->tpt_coef, 0, sizeof(ctx->tpt_coef));
       sci_tpt_pack_coeffs(F, (int)kind, pes_coeffs, gamma, ctx->tpt_coef);
       ctx->wave = (long long)ctx->sm_count * sci_tpt_blocks_per_sm(F, (int)kind) * sci_tpt_traj_per_block();
+    } else if (cml) {
+      ctx->wave = (long long)ctx->sm_count * sci_cml_traj_per_block(F);  // one CTA per SM
     } else {
       ctx->wave = (long long)ctx->sm_count * sci_prop_blocks_per_sm(F, (int)kind) * sci_prop_traj_per_block(F);
     }
@@ -541,8 +561,12 @@ sc_ivr_status sc_ivr_eval_pes(sc_ivr_ctx *ctx, const double *q, long long n, dou
     CU(sci_tpt_launch_eval_pes(ctx->F, ctx->kind, TP, q, n, V_out, g_out, H_out, (cudaStream_t)cuda_stream));
     return SC_IVR_OK;
   }
-  CU(sci_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
-                         (cudaStream_t)cuda_stream));
+  if (sci_cml_lanes(ctx->F))
+    CU(sci_cml_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
+                               (cudaStream_t)cuda_stream));
+  else
+    CU(sci_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
+                           (cudaStream_t)cuda_stream));
   return SC_IVR_OK;
 }
 

@@ -27,6 +27,11 @@ struct PropParams {
   int nstages;
   double kick[SCI_MAX_STAGES];   // b_i * dt
   double drift[SCI_MAX_STAGES];  // a_i * dt
+  // the same composition as a table of evaluation points (propagate_cml.cu): a step visits npoints positions; at point e
+  // the kicks up to the snapshot sum to pt_pre[e] (point 0 only: the end of the previous step), those after it to
+  // pt_post[e], and the drift that leaves the point is pt_drift[e]
+  int npoints;
+  double pt_pre[SCI_MAX_STAGES], pt_post[SCI_MAX_STAGES], pt_drift[SCI_MAX_STAGES];
   double sg[SCI_MAXF];           // sqrt(gamma)
   double isg[SCI_MAXF];          // 1/sqrt(gamma)
   double mu[SCI_MAXF];           // gamma/mass: dQ/dt = mu P, T = 1/2 sum mu P^2
@@ -82,6 +87,14 @@ size_t sci_pack_coeffs(int F, int kind, const double *coeffs, const double *gamm
 cudaError_t sci_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st);
 cudaError_t sci_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q,
                                 long long n, double *V, double *g, double *H, cudaStream_t st);
+
+// C-modes-per-lane kernels with the monodromy state in tensor memory (propagate_cml.cu)
+int sci_cml_lanes(int F);  // lanes per trajectory, 0 = F is not served by these kernels
+int sci_cml_traj_per_block(int F);
+size_t sci_cml_pack_coeffs(int F, int kind, const double *coeffs, const double *gamma, double *out /*may be NULL: size query*/);
+cudaError_t sci_cml_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st);
+cudaError_t sci_cml_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q,
+                                    long long n, double *V, double *g, double *H, cudaStream_t st);
 
 // thread-per-trajectory kernels (propagate_tpt.cu)
 int sci_tpt_traj_per_block();

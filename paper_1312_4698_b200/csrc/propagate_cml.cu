@@ -1,0 +1,985 @@
+// Kernel A, "C modes per lane" mapping with the monodromy state in tensor memory (rows a1-a7 of DESIGN.md).
+//
+// Mapping.  L lanes per trajectory, G = floor(32 / L) trajectories per warp, lane = l * G + g (l = lane class,
+// g = trajectory of the warp).  Lane l owns the modes a = l + s L, s = 0 .. C-1 (C = ceil(F / L)): their (P_a, Q_a), its
+// share of the action, and the 2 C tangent vectors d(P,Q)/dP0_a (slot s) and d(P,Q)/dQ0_a (slot C + s), i.e. 2 C
+// columns of the 2F x 2F monodromy matrix M.  The columns of M evolve independently given the
+// Hessian, so nothing but the Hessian and the pivot columns of the two eliminations crosses lanes.
+//
+// Where the state lives (per SM: one CTA of 8 warps):
+//   tensor memory   the lane's 2 C columns of M (4 C F doubles), exactly the matrix M(c) of the last integer time c:
+//                   TMEM is used as lane-private scratch through tcgen05.ld / tcgen05.st (32x32b), two warps per
+//                   32-lane quadrant, 128 doubles per lane each
+//   registers       the working copies of the two eliminations (a5: det 2K, complex F x F; a7: det M, real 2F x 2F)
+//   shared memory   per trajectory: Q exchange, Hessian entries, the pivot columns of the running elimination steps;
+//                   per lane: H dQ of the last evaluation point (used twice: closing kick before the snapshot, opening
+//                   kick after it)
+//
+// Per time step (velocity-Verlet; the general "kick b_s, drift a_s" composition is a table of evaluation points):
+//   snapshot  M-LU and K-LU from the TMEM state (static pivot order with look-ahead, monitored multipliers, pivoted
+//             fallback), record (ln|<chi|pq>|, S + arg<chi|pq>, det 2K), flag |det M - 1| <= tol
+//   pass      scalars kick/drift; PES at the new Q (gradient, Hessian -> shared memory); per column: opening kick with
+//             the parked H dQ, drift, new H dQ, closing kick, store to TMEM, park H dQ
+//
+// Everything runs in reduced coordinates Q = sqrt(gamma) q, P = p / sqrt(gamma): 2K = (M_qq + M_pp) + i (M_pq - M_qp).
+#include "common.cuh"
+#include "tmem_ldst.cuh"
+
+namespace {
+
+constexpr int kWarpsC = 8;
+constexpr int kThreadsC = kWarpsC * 32;
+
+__device__ __forceinline__ double rcp_nr2(double x) {
+  // MUFU.RCP64H seed (2^-23 relative) + two Newton steps: ~1 ulp for normal x, no slow path.
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  return r;
+}
+
+__device__ __forceinline__ unsigned abs_hi(double x) { return (unsigned)__double2hiint(x) & 0x7fffffffu; }
+
+template <int F, int L>
+struct Cml {
+  static constexpr int C = (F + L - 1) / L;   // modes per lane
+  static constexpr int G = 32 / L;            // trajectories per warp
+  static constexpr int ACT = G * L;           // lanes that own a trajectory share; the rest clone lane 0 and store nothing
+  static constexpr int N = 2 * F;             // rows of M: dP_0..dP_{F-1}, dQ_0..dQ_{F-1}
+  static constexpr int NS = 2 * C;            // columns (slots) of M per lane
+  static constexpr int ND = F / 2 + 1;        // Hessian entries (a, (a+d)%F), d = 0..ND-1, computed by the owner of mode a
+  static constexpr int NR = (F - 1) / 2;      // cubic-gradient terms received from the owners of modes a-d
+  static constexpr int NH = ND * F;
+  static constexpr int TCOLS = NS * N * 2;    // 32-bit TMEM columns per lane
+  static_assert(TCOLS <= 256, "state does not fit the half quadrant of tensor memory a warp owns");
+  static constexpr bool EXACT = (F % L) == 0; // no phantom modes
+  // packed coefficients.  QFF: per lane class l and slot s a list of LAP doubles, pair t of the list of (l, s) at
+  // double2 index (s * LAP/2 + t) * L + l.  Positions within a list:
+  static constexpr int L_C3 = 0;               // [ND][F]  (d, k) -> Phi~[a][(a+d)%F][k]
+  static constexpr int L_C4U = L_C3 + ND * F;  // [F]      j      -> P~[a][j]
+  static constexpr int L_C4D = L_C4U + F;      // [ND]     d      -> P~[a][(a+d)%F]
+  static constexpr int L_W2 = L_C4D + ND;      //                    omega_a^2 / gamma_a
+  static constexpr int LA = L_W2 + 1;
+  static constexpr int LAP = (LA + 1) & ~1;
+  static constexpr int NCOEF_QFF = C * LAP * L;
+  static constexpr int NCOEF_MORSE = 3 * C * L;  // (D, a~, Qe) of slot s, lane class l at ((s * 3 + j) * L + l)
+  static constexpr int NCOEF = NCOEF_QFF > NCOEF_MORSE ? NCOEF_QFF : NCOEF_MORSE;
+  static constexpr int NCOEFP = (NCOEF + 1) & ~1;
+  // per-warp shared memory, in doubles.  Group arrays are [element][G] (the L lanes of trajectory g read the same word,
+  // the G trajectories adjacent words); the parked H dQ is lane-private, [element][32].
+  static constexpr int O_QS = 0;                      // [F]
+  static constexpr int O_HS = O_QS + F * G;           // [NH]
+  static constexpr int O_G3 = O_HS + NH * G;          // [NR][F]
+  static constexpr int MBN = N;                       // doubles per monodromy pivot buffer: 1/pivot + rows k+1..N-1
+  static constexpr int O_MB = O_G3 + NR * F * G;      // [2][MBN]
+  static constexpr int KBN = 2 * F;                   // doubles per Herman-Kluk pivot buffer: 1/pivot + rows k+1..F-1, complex
+  static constexpr int O_KB = O_MB + 2 * MBN * G;     // [2][KBN]
+  static constexpr int O_RED = O_KB + 2 * KBN * G;    // [L][2]
+  static constexpr int O_HM = O_RED + 2 * L * G;      // [NS * F][32], lane-private
+  static constexpr int WS = O_HM + NS * F * 32;
+  static constexpr size_t SMEM = sizeof(double) * (NCOEFP + (size_t)kWarpsC * WS) + 16;
+
+  // column (l, s) of M: mode a = l + (s % C) L, half h = s / C (0: d/dP0_a, 1: d/dQ0_a), global index h F + a.
+  // Elimination step k uses the diagonal pivot of the column with global index k.
+  __host__ __device__ static constexpr int step_lane(int k) { return (k % F) % L; }
+  __host__ __device__ static constexpr int step_slot(int k) { return (k % F) / L + (k / F) * C; }
+  // largest global index of slot s over the lane classes (is any lane's column s still live after step k?)
+  __host__ __device__ static constexpr int slot_max_index(int s) {
+    return (s / C) * F + (((s % C) * L + L - 1) < F - 1 ? ((s % C) * L + L - 1) : F - 1);
+  }
+};
+
+// ---- a1: potential share, gradient components and Hessian entries of the lane's modes (reduced coordinates) ----------
+// QFF (BASELINE.json configs 2-5, stand-in for the fitted surfaces of PAPER.md:157):
+//   H3_ab = sum_k Phi_abk Q_k,  g3_a = 1/2 sum_b H3_ab Q_b,  u_a = sum_j P_aj Q_j^2,
+//   g4_a = Q_a (u_a/2 - P_aa Q_a^2/3),  H4_aa = u_a/2,  H4_ab = P_ab Q_a Q_b,
+//   V = sum_a Q_a (w_a^2 Q_a/2 + g3_a/3 + g4_a/4)   (Euler's theorem on the homogeneous parts).
+// Morse: y = exp(-a (Q - Q_e)), V = D (1-y)^2, g = 2 D a y (1-y), H = 2 D a^2 y (2y-1).
+// The owner of mode a computes the entries (a, (a+d)%F), d < ND, and stores them at HS[d F + a]; the cubic gradient
+// terms that belong to the modes a+d travel through G3.  Two warp barriers inside; the caller needs one more before
+// it reads HS.
+template <int F, int L, int KIND>
+__device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *gs, int l, bool act,
+                                        const double (&Q)[Cml<F, L>::C], double (&gq)[Cml<F, L>::C], double &Va) {
+  using X = Cml<F, L>;
+  constexpr int C = X::C, G = X::G;
+  Va = 0.0;
+  if (KIND == SC_IVR_PES_QFF) {
+#pragma unroll
+    for (int s = 0; s < C; s++) {
+      const int a = l + s * L;
+      if (act && (X::EXACT || a < F)) gs[X::O_QS + a * G] = Q[s];
+    }
+    __syncwarp();
+    double q[F], q2[F];
+#pragma unroll
+    for (int i = 0; i < F; i++) {
+      q[i] = gs[X::O_QS + i * G];
+      q2[i] = q[i] * q[i];
+    }
+    double s3[C], u[C], w2[C], paa[C];
+    const double2 *c2 = reinterpret_cast<const double2 *>(cs);
+#pragma unroll
+    for (int s = 0; s < C; s++) {
+      const int a = l + s * L;
+      const bool real = X::EXACT || a < F;
+      const int ae = real ? a : 0;
+      double cf[X::LAP];
+#pragma unroll
+      for (int t = 0; t < X::LAP / 2; t++) {
+        const double2 v = c2[(s * (X::LAP / 2) + t) * L + l];
+        cf[2 * t] = v.x;
+        cf[2 * t + 1] = v.y;
+      }
+      double qd[X::ND];
+      qd[0] = Q[s];
+#pragma unroll
+      for (int d = 1; d < X::ND; d++) {
+        int b = ae + d;
+        b = b >= F ? b - F : b;
+        qd[d] = gs[X::O_QS + b * G];
+      }
+      double uu = 0.0;
+#pragma unroll
+      for (int j = 0; j < F; j++) uu = fma(cf[X::L_C4U + j], q2[j], uu);
+      double h3[X::ND];
+#pragma unroll
+      for (int d = 0; d < X::ND; d++) {
+        double t = 0.0;
+#pragma unroll
+        for (int k = 0; k < F; k++) t = fma(cf[X::L_C3 + d * F + k], q[k], t);
+        h3[d] = t;
+      }
+      double t3 = 0.0;
+#pragma unroll
+      for (int d = 0; d < X::ND; d++) t3 = fma(h3[d], qd[d], t3);
+      s3[s] = t3;
+      u[s] = uu;
+      w2[s] = cf[X::L_W2];
+      paa[s] = cf[X::L_C4D];
+      if (act && real) {
+        gs[X::O_HS + (0 * F + ae) * G] = w2[s] + h3[0] + 0.5 * uu;
+#pragma unroll
+        for (int d = 1; d < X::ND; d++) {
+          int b = ae + d;
+          b = b >= F ? b - F : b;
+          gs[X::O_HS + (d * F + ae) * G] = fma(cf[X::L_C4D + d] * Q[s], qd[d], h3[d]);
+          if (d <= X::NR) gs[X::O_G3 + ((d - 1) * F + b) * G] = h3[d] * Q[s];
+        }
+      }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < C; s++) {
+      const int a = l + s * L;
+      const bool real = X::EXACT || a < F;
+      const int ae = real ? a : 0;
+      double t3 = s3[s];
+#pragma unroll
+      for (int d = 1; d <= X::NR; d++) t3 += gs[X::O_G3 + ((d - 1) * F + ae) * G];
+      const double g3 = 0.5 * t3;
+      const double g4 = Q[s] * (0.5 * u[s] - (1.0 / 3.0) * paa[s] * Q[s] * Q[s]);
+      const double gg = fma(w2[s], Q[s], g3 + g4);
+      const double vv = Q[s] * (0.5 * w2[s] * Q[s] + (1.0 / 3.0) * g3 + 0.25 * g4);
+      gq[s] = real ? gg : 0.0;
+      Va += real ? vv : 0.0;
+    }
+  } else {
+#pragma unroll
+    for (int s = 0; s < C; s++) {
+      const int a = l + s * L;
+      const bool real = X::EXACT || a < F;
+      const double D = cs[(s * 3 + 0) * L + l], at = cs[(s * 3 + 1) * L + l], Qe = cs[(s * 3 + 2) * L + l];
+      const double y = exp(-at * (Q[s] - Qe));
+      const double vv = D * (1.0 - y) * (1.0 - y);
+      gq[s] = real ? 2.0 * D * at * y * (1.0 - y) : 0.0;
+      Va += real ? vv : 0.0;
+      if (act && real) gs[X::O_HS + a * G] = 2.0 * D * at * at * y * (2.0 * y - 1.0);
+    }
+  }
+}
+
+// ---- a3 helper: HM = H dQ for NB columns at once, H from the trajectory's shared slot (entries (i, (i+d)%F) at HS[d F + i])
+template <int F, int L, int KIND, int NB>
+__device__ __forceinline__ void hessian_times(const double *gs, const double (&dQ)[NB][F], double (&HM)[NB][F]) {
+  using X = Cml<F, L>;
+  constexpr int G = X::G;
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    const double h = gs[X::O_HS + i * G];
+#pragma unroll
+    for (int c = 0; c < NB; c++) HM[c][i] = h * dQ[c][i];
+  }
+  if (KIND == SC_IVR_PES_QFF) {
+#pragma unroll
+    for (int d = 1; d < X::ND; d++) {
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        if (F % 2 == 0 && d == F / 2 && i >= F / 2) continue;  // pair (i, i+F/2) is also stored by the owner of i+F/2
+        const int j = (i + d) % F;
+        const double h = gs[X::O_HS + (d * F + i) * G];
+#pragma unroll
+        for (int c = 0; c < NB; c++) {
+          HM[c][i] = fma(h, dQ[c][j], HM[c][i]);
+          HM[c][j] = fma(h, dQ[c][i], HM[c][j]);
+        }
+      }
+    }
+  }
+}
+
+// ---- one pass over the lane's columns at a new evaluation point (a2, a3) ----------------------------------------------
+//   dP -= post * HMprev (opening kick of the point just left, H dQ parked there);  dQ += adt mu dP (drift);
+//   HM = H(Q_new) dQ;  dP -= pre * HM (kick at the new point up to the snapshot);  state -> TMEM;  HM parked.
+// Columns are handled C at a time (the slots of one half h).
+template <int F, int L, int KIND>
+__device__ __forceinline__ void pass_cml(uint32_t tm, const double *gs, double *hm, const double (&mu)[F], double post,
+                                         double adt, double pre) {
+  using X = Cml<F, L>;
+  constexpr int C = X::C, N = X::N;
+#pragma unroll
+  for (int h = 0; h < 2; h++) {
+    double st[C * N];
+    tmem_ld_f64<C * N>(tm + h * C * N * 2, st);
+    double dP[C][F], dQ[C][F], HM[C][F];
+#pragma unroll
+    for (int c = 0; c < C; c++)
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        const double hp = hm[((h * C + c) * F + i) * 32];
+        dP[c][i] = fma(-post, hp, st[c * N + i]);
+        dQ[c][i] = fma(adt * mu[i], dP[c][i], st[c * N + F + i]);
+      }
+    hessian_times<F, L, KIND, C>(gs, dQ, HM);
+#pragma unroll
+    for (int c = 0; c < C; c++)
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        st[c * N + i] = fma(-pre, HM[c][i], dP[c][i]);
+        st[c * N + F + i] = dQ[c][i];
+        hm[((h * C + c) * F + i) * 32] = HM[c][i];
+      }
+    tmem_st_f64<C * N>(tm + h * C * N * 2, st);
+  }
+}
+
+// ---- a7: det M by LU in a STATIC pivot order with look-ahead ----------------------------------------------------------
+// W[s][i]: row i of the lane's column s.  Step k eliminates row k with the diagonal pivot of the column with global
+// index k: its owner publishes (1/pivot, rows k+1..N-1 of the column) in a per-trajectory shared buffer (two buffers
+// alternate), every lane scales its row-k elements by the reciprocal and updates its live columns.  The column that
+// holds the NEXT pivot is updated first and published before the rest of the step's updates, so that the
+// reciprocal -> store -> barrier -> load chain of step k+1 runs under the bulk of step k's arithmetic.
+// No pivot search: numerical safety is monitored instead (gm = largest |multiplier| of a live column, IEEE high word);
+// the caller repeats a step whose multipliers exceed its bound with the pivoted routine.  Result on lane
+// step_lane(N-1): det M.
+template <int F, int L>
+__device__ __forceinline__ void lu_m_cml(double (&W)[Cml<F, L>::NS][2 * F], double *gs, int l, bool act, double &detM,
+                                         unsigned &gm_out) {
+  using X = Cml<F, L>;
+  constexpr int G = X::G, N = X::N, NS = X::NS, C = X::C;
+  double Rm = 1.0;
+  unsigned gm = 0u;
+  {
+    const double r0 = rcp_nr2(W[X::step_slot(0)][0]);
+    if (act && l == X::step_lane(0)) {
+      double *b = gs + X::O_MB;
+      b[0] = r0;
+#pragma unroll
+      for (int i = 1; i < N; i++) b[i * G] = W[X::step_slot(0)][i];
+    }
+  }
+  __syncwarp();
+#pragma unroll
+  for (int k = 0; k < N - 1; k++) {
+    const double *b = gs + X::O_MB + (k & 1) * X::MBN * G;
+    const double r = b[0];
+    double pc[N];
+#pragma unroll
+    for (int i = k + 1; i < N; i++) pc[i] = b[(i - k) * G];
+    Rm *= r;
+    const int sn = (k + 1 < N - 1) ? X::step_slot(k + 1) : -1;
+    if (sn >= 0) {
+      const double m = W[sn][k] * r;
+      // live on this lane: global index of (l, sn) > k
+      if ((sn / C) * F + (sn % C) * L + l > k && (X::EXACT || (sn % C) * L + l < F)) gm = max(gm, abs_hi(m));
+#pragma unroll
+      for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
+      const double rn = rcp_nr2(W[sn][k + 1]);
+      if (act && l == X::step_lane(k + 1)) {
+        double *nb = gs + X::O_MB + ((k + 1) & 1) * X::MBN * G;
+        nb[0] = rn;
+#pragma unroll
+        for (int i = k + 2; i < N; i++) nb[(i - k - 1) * G] = W[sn][i];
+      }
+      __syncwarp();
+    }
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
+      if (s == sn) continue;
+      if (X::slot_max_index(s) <= k) continue;  // dead on every lane
+      const double m = W[s][k] * r;
+      if ((s / C) * F + (s % C) * L + l > k && (X::EXACT || (s % C) * L + l < F)) gm = max(gm, abs_hi(m));
+#pragma unroll
+      for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
+    }
+  }
+  detM = W[X::step_slot(N - 1)][N - 1] * rcp_nr2(Rm);
+  gm_out = gm;
+}
+
+// ---- a5: det 2K (complex F x F; the lane's columns s = 0..C-1 are those of its modes) by the same scheme ------------------
+// Result on lane step_lane(F-1): (Dre, Dim) = det(2K) |R|^2 with R the product of the reciprocal pivots: a positive
+// multiple of det 2K; only its phase is used downstream (Eq. 10 drops |C_t|).
+template <int F, int L>
+__device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (&Ki)[Cml<F, L>::C][F], double *gs, int l,
+                                         bool act, double &Dre, double &Dim, unsigned &gk_out) {
+  using X = Cml<F, L>;
+  constexpr int G = X::G, C = X::C;
+  double Rr = 1.0, Ri = 0.0;
+  unsigned gk = 0u;
+  if (F > 1) {
+    const double pr = Kr[0][0], pi = Ki[0][0];
+    const double rn = rcp_nr2(fma(pr, pr, pi * pi));
+    if (act && l == 0) {
+      double *b = gs + X::O_KB;
+      b[0] = pr * rn;
+      b[G] = -pi * rn;
+#pragma unroll
+      for (int i = 1; i < F; i++) {
+        b[(2 * i) * G] = Kr[0][i];
+        b[(2 * i + 1) * G] = Ki[0][i];
+      }
+    }
+    __syncwarp();
+  }
+#pragma unroll
+  for (int k = 0; k < F - 1; k++) {
+    const double *b = gs + X::O_KB + (k & 1) * X::KBN * G;
+    const double rr = b[0], ri = b[G];
+    double pr[F], pi[F];
+#pragma unroll
+    for (int i = k + 1; i < F; i++) {
+      pr[i] = b[(2 * (i - k)) * G];
+      pi[i] = b[(2 * (i - k) + 1) * G];
+    }
+    {
+      const double t = Rr * rr - Ri * ri;
+      Ri = fma(Rr, ri, Ri * rr);
+      Rr = t;
+    }
+    const int sn = (k + 1 < F - 1) ? (k + 1) / L : -1;
+    if (sn >= 0) {
+      const double mr = Kr[sn][k] * rr - Ki[sn][k] * ri;
+      const double mi = fma(Kr[sn][k], ri, Ki[sn][k] * rr);
+      if (sn * L + l > k && (X::EXACT || sn * L + l < F)) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+#pragma unroll
+      for (int i = k + 1; i < F; i++) {
+        Kr[sn][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[sn][i]));
+        Ki[sn][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[sn][i]));
+      }
+      const double qr = Kr[sn][k + 1], qi = Ki[sn][k + 1];
+      const double rn = rcp_nr2(fma(qr, qr, qi * qi));
+      if (act && l == (k + 1) % L) {
+        double *nb = gs + X::O_KB + ((k + 1) & 1) * X::KBN * G;
+        nb[0] = qr * rn;
+        nb[G] = -qi * rn;
+#pragma unroll
+        for (int i = k + 2; i < F; i++) {
+          nb[(2 * (i - k - 1)) * G] = Kr[sn][i];
+          nb[(2 * (i - k - 1) + 1) * G] = Ki[sn][i];
+        }
+      }
+      __syncwarp();
+    }
+#pragma unroll
+    for (int s = 0; s < C; s++) {
+      if (s == sn) continue;
+      if ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= k) continue;
+      const double mr = Kr[s][k] * rr - Ki[s][k] * ri;
+      const double mi = fma(Kr[s][k], ri, Ki[s][k] * rr);
+      if (s * L + l > k && (X::EXACT || s * L + l < F)) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+#pragma unroll
+      for (int i = k + 1; i < F; i++) {
+        Kr[s][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[s][i]));
+        Ki[s][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[s][i]));
+      }
+    }
+  }
+  // det 2K = p_{F-1} / R  ~  p_{F-1} conj(R)
+  const double lr = Kr[(F - 1) / L][F - 1], li = Ki[(F - 1) / L][F - 1];
+  Dre = fma(lr, Rr, li * Ri);
+  Dim = fma(li, Rr, -lr * Ri);
+  gk_out = gk;
+}
+
+// ---- a5 + a7, rare path: both determinants with partial pivoting ------------------------------------------------------
+// Every lane gathers the whole matrix M(c) of its trajectory from the TMEM state of the trajectory's lanes (warp
+// shuffles) into local memory and eliminates it serially; the L lanes of a trajectory compute the same numbers.
+template <int F, int L>
+__device__ __noinline__ void pivoted_dets_cml(uint32_t tm, int g, bool with_m, double &Dre, double &Dim, double &dM) {
+  using X = Cml<F, L>;
+  constexpr int G = X::G, N = X::N, C = X::C, NS = X::NS;
+  double A[N * N];
+#pragma unroll 1
+  for (int i = 0; i < N * N; i++) A[i] = 0.0;
+#pragma unroll
+  for (int s = 0; s < NS; s++) {
+    double col[N];
+    tmem_ld_f64<N>(tm + s * N * 2, col);
+#pragma unroll
+    for (int lp = 0; lp < L; lp++) {
+      const int a = lp + (s % C) * L;
+      if (a >= F) continue;
+      const int j = (s / C) * F + a;
+#pragma unroll
+      for (int i = 0; i < N; i++) A[i * N + j] = __shfl_sync(0xffffffffu, col[i], lp * G + g);
+    }
+  }
+  // 2K = (M_qq + M_pp) + i (M_pq - M_qp), rows/columns in (P, Q) order (Eq. 5, reading R2, reduced coordinates)
+  double Br[F * F], Bi[F * F];
+#pragma unroll 1
+  for (int i = 0; i < F; i++)
+#pragma unroll 1
+    for (int a = 0; a < F; a++) {
+      Br[i * F + a] = A[(F + i) * N + F + a] + A[i * N + a];
+      Bi[i * F + a] = A[i * N + F + a] - A[(F + i) * N + a];
+    }
+  double dr = 1.0, di = 0.0;
+#pragma unroll 1
+  for (int k = 0; k < F; k++) {
+    int p = k;
+    double best = -1.0;
+#pragma unroll 1
+    for (int i = k; i < F; i++) {
+      const double m = fma(Br[i * F + k], Br[i * F + k], Bi[i * F + k] * Bi[i * F + k]);
+      if (m > best) {
+        best = m;
+        p = i;
+      }
+    }
+    if (!(best > 0.0)) {  // singular column (0) or nothing but NaN below the diagonal
+      dr = di = (best == 0.0) ? 0.0 : nan("");
+      break;
+    }
+    if (p != k) {
+#pragma unroll 1
+      for (int j = k; j < F; j++) {
+        double t = Br[k * F + j];
+        Br[k * F + j] = Br[p * F + j];
+        Br[p * F + j] = t;
+        t = Bi[k * F + j];
+        Bi[k * F + j] = Bi[p * F + j];
+        Bi[p * F + j] = t;
+      }
+      dr = -dr;
+      di = -di;
+    }
+    const double pr = Br[k * F + k], pi = Bi[k * F + k];
+    {
+      const double t = dr * pr - di * pi;
+      di = dr * pi + di * pr;
+      dr = t;
+    }
+    // keep the running product in range: only its phase is used
+    {
+      const double sc = fmax(fabs(dr), fabs(di));
+      if (sc > 0.0 && isfinite(sc)) {
+        int e;
+        frexp(sc, &e);
+        dr = ldexp(dr, -e);
+        di = ldexp(di, -e);
+      }
+    }
+    const double inv = 1.0 / best;
+#pragma unroll 1
+    for (int i = k + 1; i < F; i++) {
+      const double xr = Br[i * F + k], xi = Bi[i * F + k];
+      const double mr = (xr * pr + xi * pi) * inv, mi = (xi * pr - xr * pi) * inv;
+#pragma unroll 1
+      for (int j = k + 1; j < F; j++) {
+        const double ur = Br[k * F + j], ui = Bi[k * F + j];
+        Br[i * F + j] -= mr * ur - mi * ui;
+        Bi[i * F + j] -= mr * ui + mi * ur;
+      }
+    }
+  }
+  Dre = dr;
+  Dim = di;
+  dM = 1.0;
+  if (with_m) {
+    double det = 1.0;
+#pragma unroll 1
+    for (int k = 0; k < N; k++) {
+      int p = k;
+      double best = -1.0;
+#pragma unroll 1
+      for (int i = k; i < N; i++) {
+        const double m = fabs(A[i * N + k]);
+        if (m > best) {
+          best = m;
+          p = i;
+        }
+      }
+      if (!(best > 0.0)) {
+        det = (best == 0.0) ? 0.0 : nan("");
+        break;
+      }
+      if (p != k) {
+#pragma unroll 1
+        for (int j = k; j < N; j++) {
+          const double t = A[k * N + j];
+          A[k * N + j] = A[p * N + j];
+          A[p * N + j] = t;
+        }
+        det = -det;
+      }
+      const double pv = A[k * N + k];
+      det *= pv;
+#pragma unroll 1
+      for (int i = k + 1; i < N; i++) {
+        const double m = A[i * N + k] / pv;
+#pragma unroll 1
+        for (int j = k + 1; j < N; j++) A[i * N + j] -= m * A[k * N + j];
+      }
+    }
+    dM = det;
+  }
+}
+
+// ---- snapshot: both determinants of M(c) from the TMEM state -----------------------------------------------------------
+template <int F, int L, bool WITH_M>
+__device__ __forceinline__ void dets_cml(uint32_t tm, double *gs, int l, bool act, double &Dre, double &Dim, double &dM,
+                                         unsigned &gk, unsigned &gm) {
+  using X = Cml<F, L>;
+  constexpr int C = X::C, N = X::N, NS = X::NS;
+  dM = 1.0;
+  gm = 0u;
+  if (WITH_M) {
+    double W[NS][N];
+    {
+      double st[NS * N];
+      tmem_ld_f64<NS * N>(tm, st);
+#pragma unroll
+      for (int s = 0; s < NS; s++)
+#pragma unroll
+        for (int i = 0; i < N; i++) W[s][i] = st[s * N + i];
+    }
+    lu_m_cml<F, L>(W, gs, l, act, dM, gm);
+  }
+  double Kr[C][F], Ki[C][F];
+#pragma unroll
+  for (int s = 0; s < C; s++) {
+    double c1[N], c2[N];  // columns d/dP0_a and d/dQ0_a of the lane's mode s
+    tmem_ld_f64<N>(tm + s * N * 2, c1);
+    tmem_ld_f64<N>(tm + (C + s) * N * 2, c2);
+#pragma unroll
+    for (int i = 0; i < F; i++) {
+      Kr[s][i] = c2[F + i] + c1[i];  // dQ2 + dP1
+      Ki[s][i] = c2[i] - c1[F + i];  // dP2 - dQ1
+    }
+  }
+  lu_k_cml<F, L>(Kr, Ki, gs, l, act, Dre, Dim, gk);
+}
+
+template <int F, int L, int KIND>
+__global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_constant__ PropParams P) {
+  using X = Cml<F, L>;
+  constexpr int C = X::C, G = X::G, N = X::N, NS = X::NS;
+  extern __shared__ double smem[];
+  double *cs = smem;
+  uint32_t *tm_slot = reinterpret_cast<uint32_t *>(smem + X::NCOEFP + kWarpsC * X::WS);
+  {
+    const int nco = (KIND == SC_IVR_PES_QFF) ? X::NCOEF_QFF : X::NCOEF_MORSE;
+    for (int i = threadIdx.x; i < nco; i += kThreadsC) cs[i] = P.coef[i];
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (warp == 0) tmem_alloc_all(tm_slot);
+  tmem_fence_before_sync();
+  __syncthreads();
+  tmem_fence_after_sync();
+  const uint32_t tm_base = *tm_slot;
+  // two warps per 32-lane quadrant: warp w owns lanes 32 (w % 4) .. +31, columns 256 (w / 4) .. +255
+  const uint32_t tm = tm_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * 256);
+
+  const bool act = lane < X::ACT;
+  const int l = act ? lane / G : 0, g = act ? lane - l * G : 0;
+  double *ws = smem + X::NCOEFP + warp * X::WS;
+  double *gs = ws + g;                  // group arrays: element e at gs[O_x + e * G]
+  double *hm = ws + X::O_HM + lane;     // parked H dQ: element e at hm[e * 32]
+  unsigned gmask = 0u;
+#pragma unroll
+  for (int i = 0; i < L; i++) gmask |= 1u << (i * G + g);
+
+  const long long jj = ((long long)blockIdx.x * kWarpsC + warp) * G + g;
+  const bool valid = act && jj < P.nb;
+  const long long jl = jj < P.nb ? jj : P.nb - 1;  // tail groups recompute the last trajectory and store nothing
+  const long long jg = P.j0 + jl;
+
+  double mu[F];
+#pragma unroll
+  for (int i = 0; i < F; i++) mu[i] = P.mu[i];
+  double Pm[C], Q[C], mu_s[C], Peq_s[C], Qeq_s[C], gq[C];
+#pragma unroll
+  for (int s = 0; s < C; s++) {
+    const int a = l + s * L;
+    const bool real = X::EXACT || a < F;
+    const int ae = real ? a : 0;
+    mu_s[s] = real ? P.mu[ae] : 0.0;
+    Peq_s[s] = P.Peq[ae];
+    Qeq_s[s] = P.Qeq[ae];
+    Pm[s] = real ? P.p0q0[(long long)ae * P.stride + jg] * P.isg[ae] : Peq_s[s];
+    Q[s] = real ? P.p0q0[(long long)(F + ae) * P.stride + jg] * P.sg[ae] : Qeq_s[s];
+  }
+  double Sa = 0.0, Va;
+
+  // M(0) = 1 in TMEM; nothing parked yet
+#pragma unroll
+  for (int s = 0; s < NS; s++) {
+    double col[N];
+    const int a = l + (s % C) * L;
+#pragma unroll
+    for (int i = 0; i < N; i++) col[i] = (i == (s / C) * F + a && (X::EXACT || a < F)) ? 1.0 : 0.0;
+    tmem_st_f64<N>(tm + s * N * 2, col);
+  }
+#pragma unroll 1
+  for (int e = 0; e < NS * F; e++) hm[e * 32] = 0.0;
+  pes_cml<F, L, KIND>(cs, gs, l, act, Q, gq, Va);
+  __syncwarp();
+  pass_cml<F, L, KIND>(tm, gs, hm, mu, 0.0, 0.0, 0.0);
+
+  const int lw = X::step_lane(N - 1);  // the lane class that ends up with the last pivots of both eliminations
+  bool good = true;
+  int det_count = 0;  // steps until the next check
+  const int nsteps = P.nsteps;
+#pragma unroll 1
+  for (int c = 0;; c++) {
+    const bool last = (c == nsteps);
+    const bool check = (det_count == 0) || last;  // warp-uniform
+    // a6 (Eq. 3): the lane's share of ln<chi|pq> and of the phase S + arg<chi|pq>, at the integer time c
+    if (P.raw != nullptr) {
+      double oa = 0.0, ob = Sa;
+#pragma unroll
+      for (int s = 0; s < C; s++) {
+        if (!X::EXACT && l + s * L >= F) continue;
+        const double dq = Qeq_s[s] - Q[s], dp = Peq_s[s] - Pm[s];
+        oa = fma(-0.25, fma(dq, dq, dp * dp), oa);
+        ob = fma(0.5 * (Peq_s[s] + Pm[s]), dq, ob);
+        if (P.pq_steps != nullptr && valid)
+          P.pq_steps[((long long)c * F + (l + s * L)) * P.raw_stride + jj] = make_double2(Pm[s], Q[s]);
+      }
+      if (P.raw_plain) {  // several reference states: the record carries S alone, (P, Q) of the step go out beside it
+        oa = 0.0;
+        ob = Sa;
+      }
+      if (act) {
+        gs[X::O_RED + (2 * l) * G] = oa;
+        gs[X::O_RED + (2 * l + 1) * G] = ob;
+      }
+    }
+    double Dre, Dim, dM;
+    unsigned growK, growM;
+    if (check) dets_cml<F, L, true>(tm, gs, l, act, Dre, Dim, dM, growK, growM);
+    else dets_cml<F, L, false>(tm, gs, l, act, Dre, Dim, dM, growK, growM);
+    {
+      // static order not safe for this matrix (or forced by the caller): repeat with the pivoted eliminations
+      const bool risky = act && ((growK >= P.grow_k_max) || (check && growM >= P.grow_m_max));
+      const unsigned rb = __ballot_sync(0xffffffffu, risky);
+      if (rb != 0u) {
+        double fDre, fDim, fdM;
+        pivoted_dets_cml<F, L>(tm, g, check, fDre, fDim, fdM);
+        if ((rb & gmask) != 0u) {
+          Dre = fDre;
+          Dim = fDim;
+          dM = fdM;
+          if (P.fb_count != nullptr && l == 0 && valid) atomicAdd(P.fb_count, 1ULL);  // statistics only
+        }
+      }
+    }
+    // a8 input record, written by the lane that holds the last pivots
+    if (P.raw != nullptr) {
+      __syncwarp();
+      if (l == lw) {
+        double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+        for (int i = 0; i < L; i++) {
+          s0 += gs[X::O_RED + (2 * i) * G];
+          s1 += gs[X::O_RED + (2 * i + 1) * G];
+        }
+        // only the phase of the determinant is used: bring it to unit scale (a power of two, exact)
+        const int ex = (int)((max(abs_hi(Dre), abs_hi(Dim)) >> 20) & 0x7ffu);
+        if (ex > 0 && ex < 0x7fe) {
+          const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex): finite and normal for every ex
+          Dre *= sc;
+          Dim *= sc;
+        }
+        if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre, Dim);
+      }
+    }
+    // a7: |det M - 1| <= tol and finite, every det_stride steps and at the end
+    if (check) {
+      bool ok = (l == lw) ? (fabs(dM - 1.0) <= P.det_tol) : true;
+      ok = ok && isfinite(Sa);
+#pragma unroll
+      for (int s = 0; s < C; s++) ok = ok && isfinite(Pm[s]) && isfinite(Q[s]);
+      good = good && ok;
+      det_count = P.det_stride;
+    }
+    det_count--;
+    if (last) break;
+    // a2-a4 (R10, R11): evaluation points of the "kick b_s, drift a_s" composition
+#pragma unroll 1
+    for (int e = 0; e < P.npoints; e++) {
+      const double post = P.pt_post[e], adt = P.pt_drift[e];
+      const double pre = P.pt_pre[(e + 1 == P.npoints) ? 0 : e + 1];
+      Sa = fma(-post, Va, Sa);
+#pragma unroll
+      for (int s = 0; s < C; s++) {
+        Pm[s] = fma(-post, gq[s], Pm[s]);
+        Sa = fma(0.5 * adt * mu_s[s], Pm[s] * Pm[s], Sa);
+        Q[s] = fma(adt * mu_s[s], Pm[s], Q[s]);
+      }
+      __syncwarp();  // every lane is done with the Hessian / pivot slots of the previous point
+      pes_cml<F, L, KIND>(cs, gs, l, act, Q, gq, Va);
+      __syncwarp();
+      pass_cml<F, L, KIND>(tm, gs, hm, mu, post, adt, pre);
+      Sa = fma(-pre, Va, Sa);
+#pragma unroll
+      for (int s = 0; s < C; s++) Pm[s] = fma(-pre, gq[s], Pm[s]);
+    }
+  }
+
+  // outputs
+  const unsigned bal = __ballot_sync(0xffffffffu, good);
+  const bool group_good = ((bal & gmask) == gmask);
+  double Stot = 0.0;
+#pragma unroll
+  for (int i = 0; i < L; i++) Stot += __shfl_sync(0xffffffffu, Sa, i * G + g);
+  if (valid) {
+    if (P.good != nullptr && l == 0) P.good[jj] = group_good ? 1 : 0;
+    if (P.S_out != nullptr && l == 0) P.S_out[jg] = Stot;
+    if (P.pq_out != nullptr) {
+#pragma unroll
+      for (int s = 0; s < C; s++) {
+        const int a = l + s * L;
+        if (!X::EXACT && a >= F) continue;
+        P.pq_out[(long long)a * P.stride + jg] = Pm[s] * P.sg[a];
+        P.pq_out[(long long)(F + a) * P.stride + jg] = Q[s] * P.isg[a];
+      }
+    }
+  }
+  if (P.M_out != nullptr) {
+    // M_xy[i][a], reduced -> caller's units: p = sg P, q = Q / sg
+#pragma unroll
+    for (int s = 0; s < NS; s++) {
+      double col[N];
+      tmem_ld_f64<N>(tm + s * N * 2, col);
+      const int a = l + (s % C) * L, h = s / C;
+      if (!valid || (!X::EXACT && a >= F)) continue;
+      const double ca = h == 0 ? P.isg[a] : P.sg[a];
+      const long long blk = (long long)F * F * P.stride;
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        const long long e = ((long long)i * F + a) * P.stride + jg;
+        P.M_out[(h == 0 ? 0 : 1) * blk + e] = col[i] * P.sg[i] * ca;
+        P.M_out[(h == 0 ? 2 : 3) * blk + e] = col[F + i] * P.isg[i] * ca;
+      }
+    }
+  }
+  tmem_fence_before_sync();
+  __syncthreads();
+  if (warp == 0) tmem_free_all(tm_base);
+}
+
+// ---- debug kernel for a1: same pes_cml, caller's units out ---------------------------------------------------------------
+template <int F, int L, int KIND>
+__global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__restrict__ coef, const double *__restrict__ sgv,
+                                                            const double *__restrict__ q, long long n, double *V,
+                                                            double *gout, double *H) {
+  using X = Cml<F, L>;
+  constexpr int C = X::C, G = X::G;
+  extern __shared__ double smem[];
+  double *cs = smem;
+  {
+    const int nco = (KIND == SC_IVR_PES_QFF) ? X::NCOEF_QFF : X::NCOEF_MORSE;
+    for (int i = threadIdx.x; i < nco; i += kThreadsC) cs[i] = coef[i];
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool act = lane < X::ACT;
+  const int l = act ? lane / G : 0, g = act ? lane - l * G : 0;
+  double *gs = smem + X::NCOEFP + warp * X::WS + g;
+  const long long jj = ((long long)blockIdx.x * kWarpsC + warp) * G + g;
+  const bool valid = act && jj < n;
+  const long long jl = jj < n ? jj : n - 1;
+  double Q[C], gq[C], Va;
+#pragma unroll
+  for (int s = 0; s < C; s++) {
+    const int a = l + s * L;
+    Q[s] = (X::EXACT || a < F) ? q[(long long)a * n + jl] * sgv[a] : 0.0;
+  }
+  pes_cml<F, L, KIND>(cs, gs, l, act, Q, gq, Va);
+  __syncwarp();
+  double Vt = 0.0;
+#pragma unroll
+  for (int i = 0; i < L; i++) Vt += __shfl_sync(0xffffffffu, Va, i * G + g);
+  if (!valid) return;
+  if (l == 0) V[jl] = Vt;
+#pragma unroll
+  for (int s = 0; s < C; s++) {
+    const int a = l + s * L;
+    if (!X::EXACT && a >= F) continue;
+    gout[(long long)a * n + jl] = gq[s] * sgv[a];
+    if (KIND != SC_IVR_PES_QFF) {
+      for (int b = 0; b < F; b++) H[((long long)a * F + b) * n + jl] = (b == a) ? gs[X::O_HS + a * G] * sgv[a] * sgv[a] : 0.0;
+    } else {
+#pragma unroll
+      for (int d = 0; d < X::ND; d++) {
+        const int b = (a + d) % F;
+        const double h = gs[X::O_HS + (d * F + a) * G] * sgv[a] * sgv[b];
+        H[((long long)a * F + b) * n + jl] = h;
+        H[((long long)b * F + a) * n + jl] = h;
+      }
+    }
+  }
+}
+
+template <int F, int L, int KIND>
+cudaError_t launch_prop_cml(const PropParams &P, cudaStream_t st) {
+  using X = Cml<F, L>;
+  static int attr_dev_mask[64] = {0};  // per device: shared-memory opt-in done
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64 || !attr_dev_mask[dev]) {
+    e = cudaFuncSetAttribute(k_propagate_cml<F, L, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64) attr_dev_mask[dev] = 1;
+  }
+  const int tpb = kWarpsC * X::G;
+  const long long blocks = (P.nb + tpb - 1) / tpb;
+  k_propagate_cml<F, L, KIND><<<(unsigned)blocks, kThreadsC, X::SMEM, st>>>(P);
+  return cudaGetLastError();
+}
+
+template <int F, int L, int KIND>
+cudaError_t launch_pes_cml(const double *coef, const double *sg, const double *q, long long n, double *V, double *g, double *H,
+                           cudaStream_t st) {
+  using X = Cml<F, L>;
+  cudaError_t e = cudaFuncSetAttribute(k_eval_pes_cml<F, L, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM);
+  if (e != cudaSuccess) return e;
+  const int tpb = kWarpsC * X::G;
+  const long long blocks = (n + tpb - 1) / tpb;
+  k_eval_pes_cml<F, L, KIND><<<(unsigned)blocks, kThreadsC, X::SMEM, st>>>(coef, sg, q, n, V, g, H);
+  return cudaGetLastError();
+}
+
+// Host: reduce the caller's coefficients to the packed block of Cml<F, L>.
+//   Phi~_ijk = Phi_ijk / sqrt(g_i g_j g_k),  P~_ij = Phi_iijj / (g_i g_j),  w~_a^2 = w_a^2 / g_a   (QFF)
+//   a~ = a / sqrt(g),  Q_e = sqrt(g) q_e                                                           (Morse)
+template <int F, int L>
+size_t pack_cml(int kind, const double *c, const double *gamma, double *out) {
+  using X = Cml<F, L>;
+  constexpr int C = X::C, ND = X::ND;
+  if (kind != SC_IVR_PES_QFF) {
+    const size_t n = X::NCOEF_MORSE;
+    if (!out) return n;
+    for (size_t i = 0; i < n; i++) out[i] = 0.0;
+    for (int l = 0; l < L; l++)
+      for (int s = 0; s < C; s++) {
+        const int a = l + s * L;
+        if (a >= F) continue;
+        const double sg = sqrt(gamma[a]);
+        out[(s * 3 + 0) * L + l] = c[4 * a];
+        out[(s * 3 + 1) * L + l] = c[4 * a + 1] / sg;
+        out[(s * 3 + 2) * L + l] = c[4 * a + 2] * sg;
+      }
+    return n;
+  }
+  const size_t n = X::NCOEF_QFF;
+  if (!out) return n;
+  for (size_t i = 0; i < n; i++) out[i] = 0.0;
+  std::vector<double> phi((size_t)F * F * F, 0.0), pq((size_t)F * F, 0.0);
+  const double *cub = c + F;
+  size_t m = 0;
+  for (int i = 0; i < F; i++)
+    for (int j = i; j < F; j++)
+      for (int k = j; k < F; k++) {
+        const double v = cub[m++] / sqrt(gamma[i] * gamma[j] * gamma[k]);
+        const int p[6][3] = {{i, j, k}, {i, k, j}, {j, i, k}, {j, k, i}, {k, i, j}, {k, j, i}};
+        for (auto &t : p) phi[((size_t)t[0] * F + t[1]) * F + t[2]] = v;
+      }
+  const double *qua = cub + m;
+  m = 0;
+  for (int i = 0; i < F; i++)
+    for (int j = i; j < F; j++) {
+      const double v = qua[m++] / (gamma[i] * gamma[j]);
+      pq[i * F + j] = pq[j * F + i] = v;
+    }
+  std::vector<double> list(X::LAP);
+  for (int l = 0; l < L; l++)
+    for (int s = 0; s < C; s++) {
+      const int a = l + s * L;
+      if (a >= F) continue;
+      for (auto &x : list) x = 0.0;
+      for (int d = 0; d < ND; d++)
+        for (int k = 0; k < F; k++) list[X::L_C3 + d * F + k] = phi[((size_t)a * F + (a + d) % F) * F + k];
+      for (int j = 0; j < F; j++) list[X::L_C4U + j] = pq[a * F + j];
+      for (int d = 0; d < ND; d++) list[X::L_C4D + d] = pq[a * F + (a + d) % F];
+      list[X::L_W2] = c[a] * c[a] / gamma[a];
+      for (int i = 0; i < X::LAP; i++) out[((size_t)(s * (X::LAP / 2) + i / 2) * L + l) * 2 + (i & 1)] = list[i];
+    }
+  return n;
+}
+
+}  // namespace
+
+// (F, L) pairs served by this kernel; every other F >= 4 stays on the one-mode-per-lane kernel of propagate.cu
+#define SCI_CML_FOR_EACH(X) X(9, 3)
+
+int sci_cml_lanes(int F) {
+  switch (F) {
+#define X(f, l) case f: return l;
+    SCI_CML_FOR_EACH(X)
+#undef X
+  }
+  return 0;
+}
+
+int sci_cml_traj_per_block(int F) {
+  const int L = sci_cml_lanes(F);
+  return L ? kWarpsC * (32 / L) : 0;
+}
+
+size_t sci_cml_pack_coeffs(int F, int kind, const double *c, const double *gamma, double *out) {
+  switch (F) {
+#define X(f, l) case f: return pack_cml<f, l>(kind, c, gamma, out);
+    SCI_CML_FOR_EACH(X)
+#undef X
+  }
+  return 0;
+}
+
+cudaError_t sci_cml_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st) {
+  const bool qff = kind == SC_IVR_PES_QFF;
+  switch (F) {
+#define X(f, l) case f: return qff ? launch_prop_cml<f, l, SC_IVR_PES_QFF>(P, st) : launch_prop_cml<f, l, SC_IVR_PES_MORSE_UNCOUPLED>(P, st);
+    SCI_CML_FOR_EACH(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t sci_cml_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q, long long n,
+                                    double *V, double *g, double *H, cudaStream_t st) {
+  const bool qff = kind == SC_IVR_PES_QFF;
+  switch (F) {
+#define X(f, l) case f: return qff ? launch_pes_cml<f, l, SC_IVR_PES_QFF>(coef, sg, q, n, V, g, H, st) \
+                                   : launch_pes_cml<f, l, SC_IVR_PES_MORSE_UNCOUPLED>(coef, sg, q, n, V, g, H, st);
+    SCI_CML_FOR_EACH(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
