@@ -43,6 +43,18 @@ __device__ __forceinline__ double rcp_nr2(double x) {
 
 __device__ __forceinline__ unsigned abs_hi(double x) { return (unsigned)__double2hiint(x) & 0x7fffffffu; }
 
+// shared memory through 32-bit addresses (one base register, the offsets are immediates)
+__device__ __forceinline__ double lds(uint32_t a) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+// predicated store: lanes with own == 0 issue nothing (no branch around the owner's publications)
+__device__ __forceinline__ void sts_if(uint32_t a, double v, int own) {
+  asm volatile("{ .reg .pred p; setp.ne.s32 p, %2, 0; @p st.shared.f64 [%0], %1; }" ::"r"(a), "d"(v), "r"(own) : "memory");
+}
+
 template <int F, int L>
 struct Cml {
   static constexpr int C = (F + L - 1) / L;   // modes per lane
@@ -70,17 +82,22 @@ struct Cml {
   static constexpr int NCOEFP = (NCOEF + 1) & ~1;
   // per-warp shared memory, in doubles.  Group arrays are [element][G] (the L lanes of trajectory g read the same word,
   // the G trajectories adjacent words); the parked H dQ is lane-private, [element][32].
+  // Region A is used by the PES / pass phase (Q exchange, Hessian entries, cubic gradient terms) and, during the
+  // snapshot, by the pivot columns of the first F steps of the monodromy elimination, which are all kept (RP).
   static constexpr int O_QS = 0;                      // [F]
   static constexpr int O_HS = O_QS + F * G;           // [NH]
   static constexpr int O_G3 = O_HS + NH * G;          // [NR][F]
-  static constexpr int MBN = N;                       // doubles per monodromy pivot buffer: 1/pivot + rows k+1..N-1
-  static constexpr int O_MB = O_G3 + NR * F * G;      // [2][MBN]
-  static constexpr int KBN = 2 * F;                   // doubles per Herman-Kluk pivot buffer: 1/pivot + rows k+1..F-1, complex
-  static constexpr int O_KB = O_MB + 2 * MBN * G;     // [2][KBN]
+  static constexpr int PES_N = F + NH + NR * F;
+  static constexpr int RPN = F * N - F * (F - 1) / 2; // step k < F at offset rp(k): 1/pivot + rows k+1..N-1
+  static constexpr int O_RP = 0;
+  static constexpr int A_N = PES_N > RPN ? PES_N : RPN;
+  static constexpr int KBN = 2 * F;                   // doubles per buffer: complex 1/pivot + rows k+1..F-1 (a5), or the
+  static constexpr int O_KB = A_N * G;                // real 1/pivot + rows k+1..N-1 of a step k >= F (a7); [2][KBN]
   static constexpr int O_RED = O_KB + 2 * KBN * G;    // [L][2]
   static constexpr int O_HM = O_RED + 2 * L * G;      // [NS * F][32], lane-private
   static constexpr int WS = O_HM + NS * F * 32;
   static constexpr size_t SMEM = sizeof(double) * (NCOEFP + (size_t)kWarpsC * WS) + 16;
+  __host__ __device__ static constexpr int rp(int k) { return k * N - k * (k - 1) / 2; }
 
   // column (l, s) of M: mode a = l + (s % C) L, half h = s / C (0: d/dP0_a, 1: d/dQ0_a), global index h F + a.
   // Elimination step k uses the diagonal pivot of the column with global index k.
@@ -100,9 +117,9 @@ struct Cml {
 // Morse: y = exp(-a (Q - Q_e)), V = D (1-y)^2, g = 2 D a y (1-y), H = 2 D a^2 y (2y-1).
 // The owner of mode a computes the entries (a, (a+d)%F), d < ND, and stores them at HS[d F + a]; the cubic gradient
 // terms that belong to the modes a+d travel through G3.  Two warp barriers inside; the caller needs one more before
-// it reads HS.
+// it reads HS.  gsa: shared address of the trajectory's group arrays (element e of array O at gsa + 8 (O + e G)).
 template <int F, int L, int KIND>
-__device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *gs, int l, bool act,
+__device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t gsa, int l, bool act,
                                         const double (&Q)[Cml<F, L>::C], double (&gq)[Cml<F, L>::C], double &Va) {
   using X = Cml<F, L>;
   constexpr int C = X::C, G = X::G;
@@ -111,13 +128,13 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *g
 #pragma unroll
     for (int s = 0; s < C; s++) {
       const int a = l + s * L;
-      if (act && (X::EXACT || a < F)) gs[X::O_QS + a * G] = Q[s];
+      sts_if(gsa + 8 * (X::O_QS + a * G), Q[s], act && (X::EXACT || a < F));
     }
     __syncwarp();
     double q[F], q2[F];
 #pragma unroll
     for (int i = 0; i < F; i++) {
-      q[i] = gs[X::O_QS + i * G];
+      q[i] = lds(gsa + 8 * (X::O_QS + i * G));
       q2[i] = q[i] * q[i];
     }
     double s3[C], u[C], w2[C], paa[C];
@@ -127,6 +144,7 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *g
       const int a = l + s * L;
       const bool real = X::EXACT || a < F;
       const int ae = real ? a : 0;
+      const int own = act && real;
       double cf[X::LAP];
 #pragma unroll
       for (int t = 0; t < X::LAP / 2; t++) {
@@ -140,7 +158,7 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *g
       for (int d = 1; d < X::ND; d++) {
         int b = ae + d;
         b = b >= F ? b - F : b;
-        qd[d] = gs[X::O_QS + b * G];
+        qd[d] = lds(gsa + 8 * (X::O_QS + b * G));
       }
       double uu = 0.0;
 #pragma unroll
@@ -160,15 +178,13 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *g
       u[s] = uu;
       w2[s] = cf[X::L_W2];
       paa[s] = cf[X::L_C4D];
-      if (act && real) {
-        gs[X::O_HS + (0 * F + ae) * G] = w2[s] + h3[0] + 0.5 * uu;
+      sts_if(gsa + 8 * (X::O_HS + ae * G), w2[s] + h3[0] + 0.5 * uu, own);
 #pragma unroll
-        for (int d = 1; d < X::ND; d++) {
-          int b = ae + d;
-          b = b >= F ? b - F : b;
-          gs[X::O_HS + (d * F + ae) * G] = fma(cf[X::L_C4D + d] * Q[s], qd[d], h3[d]);
-          if (d <= X::NR) gs[X::O_G3 + ((d - 1) * F + b) * G] = h3[d] * Q[s];
-        }
+      for (int d = 1; d < X::ND; d++) {
+        int b = ae + d;
+        b = b >= F ? b - F : b;
+        sts_if(gsa + 8 * (X::O_HS + (d * F + ae) * G), fma(cf[X::L_C4D + d] * Q[s], qd[d], h3[d]), own);
+        if (d <= X::NR) sts_if(gsa + 8 * (X::O_G3 + ((d - 1) * F + b) * G), h3[d] * Q[s], own);
       }
     }
     __syncwarp();
@@ -179,7 +195,7 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *g
       const int ae = real ? a : 0;
       double t3 = s3[s];
 #pragma unroll
-      for (int d = 1; d <= X::NR; d++) t3 += gs[X::O_G3 + ((d - 1) * F + ae) * G];
+      for (int d = 1; d <= X::NR; d++) t3 += lds(gsa + 8 * (X::O_G3 + ((d - 1) * F + ae) * G));
       const double g3 = 0.5 * t3;
       const double g4 = Q[s] * (0.5 * u[s] - (1.0 / 3.0) * paa[s] * Q[s] * Q[s]);
       const double gg = fma(w2[s], Q[s], g3 + g4);
@@ -197,19 +213,19 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, double *g
       const double vv = D * (1.0 - y) * (1.0 - y);
       gq[s] = real ? 2.0 * D * at * y * (1.0 - y) : 0.0;
       Va += real ? vv : 0.0;
-      if (act && real) gs[X::O_HS + a * G] = 2.0 * D * at * at * y * (2.0 * y - 1.0);
+      sts_if(gsa + 8 * (X::O_HS + (real ? a : 0) * G), 2.0 * D * at * at * y * (2.0 * y - 1.0), act && real);
     }
   }
 }
 
 // ---- a3 helper: HM = H dQ for NB columns at once, H from the trajectory's shared slot (entries (i, (i+d)%F) at HS[d F + i])
 template <int F, int L, int KIND, int NB>
-__device__ __forceinline__ void hessian_times(const double *gs, const double (&dQ)[NB][F], double (&HM)[NB][F]) {
+__device__ __forceinline__ void hessian_times(uint32_t gsa, const double (&dQ)[NB][F], double (&HM)[NB][F]) {
   using X = Cml<F, L>;
   constexpr int G = X::G;
 #pragma unroll
   for (int i = 0; i < F; i++) {
-    const double h = gs[X::O_HS + i * G];
+    const double h = lds(gsa + 8 * (X::O_HS + i * G));
 #pragma unroll
     for (int c = 0; c < NB; c++) HM[c][i] = h * dQ[c][i];
   }
@@ -220,7 +236,7 @@ __device__ __forceinline__ void hessian_times(const double *gs, const double (&d
       for (int i = 0; i < F; i++) {
         if (F % 2 == 0 && d == F / 2 && i >= F / 2) continue;  // pair (i, i+F/2) is also stored by the owner of i+F/2
         const int j = (i + d) % F;
-        const double h = gs[X::O_HS + (d * F + i) * G];
+        const double h = lds(gsa + 8 * (X::O_HS + (d * F + i) * G));
 #pragma unroll
         for (int c = 0; c < NB; c++) {
           HM[c][i] = fma(h, dQ[c][j], HM[c][i]);
@@ -234,9 +250,10 @@ __device__ __forceinline__ void hessian_times(const double *gs, const double (&d
 // ---- one pass over the lane's columns at a new evaluation point (a2, a3) ----------------------------------------------
 //   dP -= post * HMprev (opening kick of the point just left, H dQ parked there);  dQ += adt mu dP (drift);
 //   HM = H(Q_new) dQ;  dP -= pre * HM (kick at the new point up to the snapshot);  state -> TMEM;  HM parked.
-// Columns are handled C at a time (the slots of one half h).
+// Columns are handled C at a time (the slots of one half h).  hma: shared address of the lane's parked H dQ
+// (element e at hma + 256 e).
 template <int F, int L, int KIND>
-__device__ __forceinline__ void pass_cml(uint32_t tm, const double *gs, double *hm, const double (&mu)[F], double post,
+__device__ __forceinline__ void pass_cml(uint32_t tm, uint32_t gsa, uint32_t hma, const PropParams &P, double post,
                                          double adt, double pre) {
   using X = Cml<F, L>;
   constexpr int C = X::C, N = X::N;
@@ -249,84 +266,163 @@ __device__ __forceinline__ void pass_cml(uint32_t tm, const double *gs, double *
     for (int c = 0; c < C; c++)
 #pragma unroll
       for (int i = 0; i < F; i++) {
-        const double hp = hm[((h * C + c) * F + i) * 32];
+        const double hp = lds(hma + 256 * ((h * C + c) * F + i));
         dP[c][i] = fma(-post, hp, st[c * N + i]);
-        dQ[c][i] = fma(adt * mu[i], dP[c][i], st[c * N + F + i]);
+        dQ[c][i] = fma(adt * P.mu[i], dP[c][i], st[c * N + F + i]);
       }
-    hessian_times<F, L, KIND, C>(gs, dQ, HM);
+    hessian_times<F, L, KIND, C>(gsa, dQ, HM);
 #pragma unroll
     for (int c = 0; c < C; c++)
 #pragma unroll
       for (int i = 0; i < F; i++) {
         st[c * N + i] = fma(-pre, HM[c][i], dP[c][i]);
         st[c * N + F + i] = dQ[c][i];
-        hm[((h * C + c) * F + i) * 32] = HM[c][i];
+        sts(hma + 256 * ((h * C + c) * F + i), HM[c][i]);
       }
     tmem_st_f64<C * N>(tm + h * C * N * 2, st);
   }
 }
 
-// ---- a7: det M by LU in a STATIC pivot order with look-ahead ----------------------------------------------------------
-// W[s][i]: row i of the lane's column s.  Step k eliminates row k with the diagonal pivot of the column with global
-// index k: its owner publishes (1/pivot, rows k+1..N-1 of the column) in a per-trajectory shared buffer (two buffers
-// alternate), every lane scales its row-k elements by the reciprocal and updates its live columns.  The column that
-// holds the NEXT pivot is updated first and published before the rest of the step's updates, so that the
+// ---- a7: det M by LU in a STATIC pivot order, in two column halves, with look-ahead ---------------------------------------
+// W[s][i]: row i of column s of the half in registers.  Step k eliminates row k with the diagonal pivot of the column
+// with global index k: its owner publishes (1/pivot, rows k+1..N-1 of the column) in the trajectory's shared slot,
+// every lane scales its row-k elements by the reciprocal and updates its live columns.  The column that holds the
+// NEXT pivot is updated first and published before the rest of the step's updates, so that the
 // reciprocal -> store -> barrier -> load chain of step k+1 runs under the bulk of step k's arithmetic.
-// No pivot search: numerical safety is monitored instead (gm = largest |multiplier| of a live column, IEEE high word);
-// the caller repeats a step whose multipliers exceed its bound with the pivoted routine.  Result on lane
-// step_lane(N-1): det M.
+// Halves: steps 0..F-1 (pivots in the d/dP0 columns) touch only the d/dP0 columns while their pivot columns are all
+// KEPT in shared memory (region RP); then the d/dQ0 columns are loaded, catch up on those F steps without any
+// barrier, and steps F..N-2 run among them (buffers in KB).  Same arithmetic as the one-piece elimination, half the
+// registers.  No pivot search: numerical safety is monitored instead (gm = largest |multiplier| of a live column,
+// IEEE high word); the caller repeats a step whose multipliers exceed its bound with the pivoted routine.
+// Result on lane step_lane(N-1): det M.
 template <int F, int L>
-__device__ __forceinline__ void lu_m_cml(double (&W)[Cml<F, L>::NS][2 * F], double *gs, int l, bool act, double &detM,
-                                         unsigned &gm_out) {
+__device__ __forceinline__ void lu_m_cml(uint32_t tm, uint32_t gsa, int l, bool act, double &detM, unsigned &gm_out) {
   using X = Cml<F, L>;
-  constexpr int G = X::G, N = X::N, NS = X::NS, C = X::C;
+  constexpr int G = X::G, N = X::N, C = X::C;
   double Rm = 1.0;
   unsigned gm = 0u;
   {
-    const double r0 = rcp_nr2(W[X::step_slot(0)][0]);
-    if (act && l == X::step_lane(0)) {
-      double *b = gs + X::O_MB;
-      b[0] = r0;
+    double W[C][N];
+    {
+      double st[C * N];
+      tmem_ld_f64<C * N>(tm, st);
 #pragma unroll
-      for (int i = 1; i < N; i++) b[i * G] = W[X::step_slot(0)][i];
+      for (int s = 0; s < C; s++)
+#pragma unroll
+        for (int i = 0; i < N; i++) W[s][i] = st[s * N + i];
+    }
+    {
+      const double r0 = rcp_nr2(W[0][0]);
+      const int own = act && l == 0;
+      sts_if(gsa + 8 * (X::O_RP + 0), r0, own);
+#pragma unroll
+      for (int i = 1; i < N; i++) sts_if(gsa + 8 * (X::O_RP + i * G), W[0][i], own);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < F; k++) {
+      const uint32_t b = gsa + 8 * (X::O_RP + X::rp(k) * G);
+      const double r = lds(b);
+      double pc[N];
+#pragma unroll
+      for (int i = k + 1; i < N; i++) pc[i] = lds(b + 8 * (i - k) * G);
+      Rm *= r;
+      const int sn = (k + 1 < F) ? (k + 1) / L : -1;
+      if (sn >= 0) {
+        const double m = W[sn][k] * r;
+        if (sn * L + l > k && (X::EXACT || sn * L + l < F)) gm = max(gm, abs_hi(m));
+#pragma unroll
+        for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
+        const double rn = rcp_nr2(W[sn][k + 1]);
+        const int own = act && l == (k + 1) % L;
+        const uint32_t nb = gsa + 8 * (X::O_RP + X::rp(k + 1) * G);
+        sts_if(nb, rn, own);
+#pragma unroll
+        for (int i = k + 2; i < N; i++) sts_if(nb + 8 * (i - k - 1) * G, W[sn][i], own);
+        __syncwarp();
+      }
+#pragma unroll
+      for (int s = 0; s < C; s++) {
+        if (s == sn) continue;
+        if ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= k) continue;  // dead on every lane
+        const double m = W[s][k] * r;
+        if (s * L + l > k && (X::EXACT || s * L + l < F)) gm = max(gm, abs_hi(m));
+#pragma unroll
+        for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
+      }
     }
   }
-  __syncwarp();
+  {
+    double W[C][N];  // the d/dQ0 columns: global index F + s L + l
+    {
+      double st[C * N];
+      tmem_ld_f64<C * N>(tm + C * N * 2, st);
 #pragma unroll
-  for (int k = 0; k < N - 1; k++) {
-    const double *b = gs + X::O_MB + (k & 1) * X::MBN * G;
-    const double r = b[0];
-    double pc[N];
+      for (int s = 0; s < C; s++)
 #pragma unroll
-    for (int i = k + 1; i < N; i++) pc[i] = b[(i - k) * G];
-    Rm *= r;
-    const int sn = (k + 1 < N - 1) ? X::step_slot(k + 1) : -1;
-    if (sn >= 0) {
-      const double m = W[sn][k] * r;
-      // live on this lane: global index of (l, sn) > k
-      if ((sn / C) * F + (sn % C) * L + l > k && (X::EXACT || (sn % C) * L + l < F)) gm = max(gm, abs_hi(m));
+        for (int i = 0; i < N; i++) W[s][i] = st[s * N + i];
+    }
+    // catch up on steps 0..F-1 (every column of this half is live during them)
 #pragma unroll
-      for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
-      const double rn = rcp_nr2(W[sn][k + 1]);
-      if (act && l == X::step_lane(k + 1)) {
-        double *nb = gs + X::O_MB + ((k + 1) & 1) * X::MBN * G;
-        nb[0] = rn;
+    for (int k = 0; k < F; k++) {
+      const uint32_t b = gsa + 8 * (X::O_RP + X::rp(k) * G);
+      const double r = lds(b);
+      double m[C];
 #pragma unroll
-        for (int i = k + 2; i < N; i++) nb[(i - k - 1) * G] = W[sn][i];
+      for (int s = 0; s < C; s++) {
+        m[s] = W[s][k] * r;
+        if (X::EXACT || s * L + l < F) gm = max(gm, abs_hi(m[s]));
       }
+#pragma unroll
+      for (int i = k + 1; i < N; i++) {
+        const double x = lds(b + 8 * (i - k) * G);
+#pragma unroll
+        for (int s = 0; s < C; s++) W[s][i] = fma(-m[s], x, W[s][i]);
+      }
+    }
+    // steps F..N-2 among the d/dQ0 columns; step k's buffer is KB[(k - F) & 1]: 1/pivot + rows k+1..N-1
+    if (F > 1) {
+      const double r0 = rcp_nr2(W[0][F]);
+      const int own = act && l == 0;
+      sts_if(gsa + 8 * (X::O_KB + 0), r0, own);
+#pragma unroll
+      for (int i = F + 1; i < N; i++) sts_if(gsa + 8 * (X::O_KB + (i - F) * G), W[0][i], own);
       __syncwarp();
     }
 #pragma unroll
-    for (int s = 0; s < NS; s++) {
-      if (s == sn) continue;
-      if (X::slot_max_index(s) <= k) continue;  // dead on every lane
-      const double m = W[s][k] * r;
-      if ((s / C) * F + (s % C) * L + l > k && (X::EXACT || (s % C) * L + l < F)) gm = max(gm, abs_hi(m));
+    for (int k = F; k < N - 1; k++) {
+      const uint32_t b = gsa + 8 * (X::O_KB + ((k - F) & 1) * X::KBN * G);
+      const double r = lds(b);
+      double pc[N];
 #pragma unroll
-      for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
+      for (int i = k + 1; i < N; i++) pc[i] = lds(b + 8 * (i - k) * G);
+      Rm *= r;
+      const int sn = (k + 1 < N - 1) ? (k + 1 - F) / L : -1;
+      if (sn >= 0) {
+        const double m = W[sn][k] * r;
+        if (F + sn * L + l > k && (X::EXACT || sn * L + l < F)) gm = max(gm, abs_hi(m));
+#pragma unroll
+        for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
+        const double rn = rcp_nr2(W[sn][k + 1]);
+        const int own = act && l == (k + 1 - F) % L;
+        const uint32_t nb = gsa + 8 * (X::O_KB + ((k + 1 - F) & 1) * X::KBN * G);
+        sts_if(nb, rn, own);
+#pragma unroll
+        for (int i = k + 2; i < N; i++) sts_if(nb + 8 * (i - k - 1) * G, W[sn][i], own);
+        __syncwarp();
+      }
+#pragma unroll
+      for (int s = 0; s < C; s++) {
+        if (s == sn) continue;
+        if (F + (s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= k) continue;
+        const double m = W[s][k] * r;
+        if (F + s * L + l > k && (X::EXACT || s * L + l < F)) gm = max(gm, abs_hi(m));
+#pragma unroll
+        for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
+      }
     }
+    detM = W[(F - 1) / L][N - 1] * rcp_nr2(Rm);
   }
-  detM = W[X::step_slot(N - 1)][N - 1] * rcp_nr2(Rm);
   gm_out = gm;
 }
 
@@ -334,7 +430,7 @@ __device__ __forceinline__ void lu_m_cml(double (&W)[Cml<F, L>::NS][2 * F], doub
 // Result on lane step_lane(F-1): (Dre, Dim) = det(2K) |R|^2 with R the product of the reciprocal pivots: a positive
 // multiple of det 2K; only its phase is used downstream (Eq. 10 drops |C_t|).
 template <int F, int L>
-__device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (&Ki)[Cml<F, L>::C][F], double *gs, int l,
+__device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (&Ki)[Cml<F, L>::C][F], uint32_t gsa, int l,
                                          bool act, double &Dre, double &Dim, unsigned &gk_out) {
   using X = Cml<F, L>;
   constexpr int G = X::G, C = X::C;
@@ -343,27 +439,26 @@ __device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (
   if (F > 1) {
     const double pr = Kr[0][0], pi = Ki[0][0];
     const double rn = rcp_nr2(fma(pr, pr, pi * pi));
-    if (act && l == 0) {
-      double *b = gs + X::O_KB;
-      b[0] = pr * rn;
-      b[G] = -pi * rn;
+    const int own = act && l == 0;
+    const uint32_t b = gsa + 8 * X::O_KB;
+    sts_if(b, pr * rn, own);
+    sts_if(b + 8 * G, -pi * rn, own);
 #pragma unroll
-      for (int i = 1; i < F; i++) {
-        b[(2 * i) * G] = Kr[0][i];
-        b[(2 * i + 1) * G] = Ki[0][i];
-      }
+    for (int i = 1; i < F; i++) {
+      sts_if(b + 8 * (2 * i) * G, Kr[0][i], own);
+      sts_if(b + 8 * (2 * i + 1) * G, Ki[0][i], own);
     }
     __syncwarp();
   }
 #pragma unroll
   for (int k = 0; k < F - 1; k++) {
-    const double *b = gs + X::O_KB + (k & 1) * X::KBN * G;
-    const double rr = b[0], ri = b[G];
+    const uint32_t b = gsa + 8 * (X::O_KB + (k & 1) * X::KBN * G);
+    const double rr = lds(b), ri = lds(b + 8 * G);
     double pr[F], pi[F];
 #pragma unroll
     for (int i = k + 1; i < F; i++) {
-      pr[i] = b[(2 * (i - k)) * G];
-      pi[i] = b[(2 * (i - k) + 1) * G];
+      pr[i] = lds(b + 8 * (2 * (i - k)) * G);
+      pi[i] = lds(b + 8 * (2 * (i - k) + 1) * G);
     }
     {
       const double t = Rr * rr - Ri * ri;
@@ -382,15 +477,14 @@ __device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (
       }
       const double qr = Kr[sn][k + 1], qi = Ki[sn][k + 1];
       const double rn = rcp_nr2(fma(qr, qr, qi * qi));
-      if (act && l == (k + 1) % L) {
-        double *nb = gs + X::O_KB + ((k + 1) & 1) * X::KBN * G;
-        nb[0] = qr * rn;
-        nb[G] = -qi * rn;
+      const int own = act && l == (k + 1) % L;
+      const uint32_t nb = gsa + 8 * (X::O_KB + ((k + 1) & 1) * X::KBN * G);
+      sts_if(nb, qr * rn, own);
+      sts_if(nb + 8 * G, -qi * rn, own);
 #pragma unroll
-        for (int i = k + 2; i < F; i++) {
-          nb[(2 * (i - k - 1)) * G] = Kr[sn][i];
-          nb[(2 * (i - k - 1) + 1) * G] = Ki[sn][i];
-        }
+      for (int i = k + 2; i < F; i++) {
+        sts_if(nb + 8 * (2 * (i - k - 1)) * G, Kr[sn][i], own);
+        sts_if(nb + 8 * (2 * (i - k - 1) + 1) * G, Ki[sn][i], own);
       }
       __syncwarp();
     }
@@ -551,23 +645,16 @@ __device__ __noinline__ void pivoted_dets_cml(uint32_t tm, int g, bool with_m, d
 
 // ---- snapshot: both determinants of M(c) from the TMEM state -----------------------------------------------------------
 template <int F, int L, bool WITH_M>
-__device__ __forceinline__ void dets_cml(uint32_t tm, double *gs, int l, bool act, double &Dre, double &Dim, double &dM,
+__device__ __forceinline__ void dets_cml(uint32_t tm, uint32_t gsa, int l, bool act, double &Dre, double &Dim, double &dM,
                                          unsigned &gk, unsigned &gm) {
   using X = Cml<F, L>;
-  constexpr int C = X::C, N = X::N, NS = X::NS;
+  constexpr int C = X::C, N = X::N;
   dM = 1.0;
   gm = 0u;
+  __syncwarp();  // region A changes hands: every lane is done with the Hessian slot of the pass
   if (WITH_M) {
-    double W[NS][N];
-    {
-      double st[NS * N];
-      tmem_ld_f64<NS * N>(tm, st);
-#pragma unroll
-      for (int s = 0; s < NS; s++)
-#pragma unroll
-        for (int i = 0; i < N; i++) W[s][i] = st[s * N + i];
-    }
-    lu_m_cml<F, L>(W, gs, l, act, dM, gm);
+    lu_m_cml<F, L>(tm, gsa, l, act, dM, gm);
+    __syncwarp();  // KB changes hands
   }
   double Kr[C][F], Ki[C][F];
 #pragma unroll
@@ -581,7 +668,7 @@ __device__ __forceinline__ void dets_cml(uint32_t tm, double *gs, int l, bool ac
       Ki[s][i] = c2[i] - c1[F + i];  // dP2 - dQ1
     }
   }
-  lu_k_cml<F, L>(Kr, Ki, gs, l, act, Dre, Dim, gk);
+  lu_k_cml<F, L>(Kr, Ki, gsa, l, act, Dre, Dim, gk);
 }
 
 template <int F, int L, int KIND>
@@ -607,8 +694,8 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
   const bool act = lane < X::ACT;
   const int l = act ? lane / G : 0, g = act ? lane - l * G : 0;
   double *ws = smem + X::NCOEFP + warp * X::WS;
-  double *gs = ws + g;                  // group arrays: element e at gs[O_x + e * G]
-  double *hm = ws + X::O_HM + lane;     // parked H dQ: element e at hm[e * 32]
+  const uint32_t gsa = (uint32_t)__cvta_generic_to_shared(ws + g);                // group arrays
+  const uint32_t hma = (uint32_t)__cvta_generic_to_shared(ws + X::O_HM + lane);   // parked H dQ
   unsigned gmask = 0u;
 #pragma unroll
   for (int i = 0; i < L; i++) gmask |= 1u << (i * G + g);
@@ -618,9 +705,6 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
   const long long jl = jj < P.nb ? jj : P.nb - 1;  // tail groups recompute the last trajectory and store nothing
   const long long jg = P.j0 + jl;
 
-  double mu[F];
-#pragma unroll
-  for (int i = 0; i < F; i++) mu[i] = P.mu[i];
   double Pm[C], Q[C], mu_s[C], Peq_s[C], Qeq_s[C], gq[C];
 #pragma unroll
   for (int s = 0; s < C; s++) {
@@ -645,10 +729,10 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     tmem_st_f64<N>(tm + s * N * 2, col);
   }
 #pragma unroll 1
-  for (int e = 0; e < NS * F; e++) hm[e * 32] = 0.0;
-  pes_cml<F, L, KIND>(cs, gs, l, act, Q, gq, Va);
+  for (int e = 0; e < NS * F; e++) sts(hma + 256 * e, 0.0);
+  pes_cml<F, L, KIND>(cs, gsa, l, act, Q, gq, Va);
   __syncwarp();
-  pass_cml<F, L, KIND>(tm, gs, hm, mu, 0.0, 0.0, 0.0);
+  pass_cml<F, L, KIND>(tm, gsa, hma, P, 0.0, 0.0, 0.0);
 
   const int lw = X::step_lane(N - 1);  // the lane class that ends up with the last pivots of both eliminations
   bool good = true;
@@ -674,15 +758,13 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         oa = 0.0;
         ob = Sa;
       }
-      if (act) {
-        gs[X::O_RED + (2 * l) * G] = oa;
-        gs[X::O_RED + (2 * l + 1) * G] = ob;
-      }
+      sts_if(gsa + 8 * (X::O_RED + (2 * l) * G), oa, act);
+      sts_if(gsa + 8 * (X::O_RED + (2 * l + 1) * G), ob, act);
     }
     double Dre, Dim, dM;
     unsigned growK, growM;
-    if (check) dets_cml<F, L, true>(tm, gs, l, act, Dre, Dim, dM, growK, growM);
-    else dets_cml<F, L, false>(tm, gs, l, act, Dre, Dim, dM, growK, growM);
+    if (check) dets_cml<F, L, true>(tm, gsa, l, act, Dre, Dim, dM, growK, growM);
+    else dets_cml<F, L, false>(tm, gsa, l, act, Dre, Dim, dM, growK, growM);
     {
       // static order not safe for this matrix (or forced by the caller): repeat with the pivoted eliminations
       const bool risky = act && ((growK >= P.grow_k_max) || (check && growM >= P.grow_m_max));
@@ -705,13 +787,13 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         double s0 = 0.0, s1 = 0.0;
 #pragma unroll
         for (int i = 0; i < L; i++) {
-          s0 += gs[X::O_RED + (2 * i) * G];
-          s1 += gs[X::O_RED + (2 * i + 1) * G];
+          s0 += lds(gsa + 8 * (X::O_RED + (2 * i) * G));
+          s1 += lds(gsa + 8 * (X::O_RED + (2 * i + 1) * G));
         }
         // only the phase of the determinant is used: bring it to unit scale (a power of two, exact)
         const int ex = (int)((max(abs_hi(Dre), abs_hi(Dim)) >> 20) & 0x7ffu);
         if (ex > 0 && ex < 0x7fe) {
-          const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex): finite and normal for every ex
+          const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex)
           Dre *= sc;
           Dim *= sc;
         }
@@ -741,10 +823,10 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         Sa = fma(0.5 * adt * mu_s[s], Pm[s] * Pm[s], Sa);
         Q[s] = fma(adt * mu_s[s], Pm[s], Q[s]);
       }
-      __syncwarp();  // every lane is done with the Hessian / pivot slots of the previous point
-      pes_cml<F, L, KIND>(cs, gs, l, act, Q, gq, Va);
+      __syncwarp();  // region A changes hands: every lane is done with the pivot columns / the previous Hessian
+      pes_cml<F, L, KIND>(cs, gsa, l, act, Q, gq, Va);
       __syncwarp();
-      pass_cml<F, L, KIND>(tm, gs, hm, mu, post, adt, pre);
+      pass_cml<F, L, KIND>(tm, gsa, hma, P, post, adt, pre);
       Sa = fma(-pre, Va, Sa);
 #pragma unroll
       for (int s = 0; s < C; s++) Pm[s] = fma(-pre, gq[s], Pm[s]);
@@ -811,6 +893,7 @@ __global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__rest
   const bool act = lane < X::ACT;
   const int l = act ? lane / G : 0, g = act ? lane - l * G : 0;
   double *gs = smem + X::NCOEFP + warp * X::WS + g;
+  const uint32_t gsa = (uint32_t)__cvta_generic_to_shared(gs);
   const long long jj = ((long long)blockIdx.x * kWarpsC + warp) * G + g;
   const bool valid = act && jj < n;
   const long long jl = jj < n ? jj : n - 1;
@@ -820,7 +903,7 @@ __global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__rest
     const int a = l + s * L;
     Q[s] = (X::EXACT || a < F) ? q[(long long)a * n + jl] * sgv[a] : 0.0;
   }
-  pes_cml<F, L, KIND>(cs, gs, l, act, Q, gq, Va);
+  pes_cml<F, L, KIND>(cs, gsa, l, act, Q, gq, Va);
   __syncwarp();
   double Vt = 0.0;
 #pragma unroll
