@@ -296,7 +296,8 @@ __device__ __forceinline__ void pass_cml(uint32_t tm, uint32_t gsa, uint32_t hma
 // IEEE high word); the caller repeats a step whose multipliers exceed its bound with the pivoted routine.
 // Result on lane step_lane(N-1): det M.
 template <int F, int L>
-__device__ __forceinline__ void lu_m_cml(uint32_t tm, uint32_t gsa, int l, bool act, double &detM, unsigned &gm_out) {
+__device__ __forceinline__ void lu_mk_cml(uint32_t tm, uint32_t gsa, int l, bool act, double &detM, unsigned &gm_out,
+                                          double &Dre, double &Dim, unsigned &gk_out) {
   using X = Cml<F, L>;
   constexpr int G = X::G, N = X::N, C = X::C;
   double Rm = 1.0;
@@ -380,48 +381,128 @@ __device__ __forceinline__ void lu_m_cml(uint32_t tm, uint32_t gsa, int l, bool 
         for (int s = 0; s < C; s++) W[s][i] = fma(-m[s], x, W[s][i]);
       }
     }
-    // steps F..N-2 among the d/dQ0 columns; step k's buffer is KB[(k - F) & 1]: 1/pivot + rows k+1..N-1
-    if (F > 1) {
-      const double r0 = rcp_nr2(W[0][F]);
-      const int own = act && l == 0;
-      sts_if(gsa + 8 * (X::O_KB + 0), r0, own);
+    // the lane's columns of 2K = (M_qq + M_pp) + i (M_pq - M_qp) (Eq. 5, reading R2, reduced coordinates)
+    double Kr[C][F], Ki[C][F];
 #pragma unroll
-      for (int i = F + 1; i < N; i++) sts_if(gsa + 8 * (X::O_KB + (i - F) * G), W[0][i], own);
+    for (int s = 0; s < C; s++) {
+      double c1[N], c2[N];  // columns d/dP0_a and d/dQ0_a of the lane's mode s
+      tmem_ld_f64<N>(tm + s * N * 2, c1);
+      tmem_ld_f64<N>(tm + (C + s) * N * 2, c2);
+#pragma unroll
+      for (int i = 0; i < F; i++) {
+        Kr[s][i] = c2[F + i] + c1[i];  // dQ2 + dP1
+        Ki[s][i] = c2[i] - c1[F + i];  // dP2 - dQ1
+      }
+    }
+    // steps F..N-2 among the d/dQ0 columns run TOGETHER with the F-1 steps of the complex elimination of 2K: two
+    // independent pivot chains per barrier.  Monodromy step k = F + j: buffer M2[j & 1] (the tail of region A, free once
+    // every lane has caught up), 1/pivot + rows k+1..N-1; Herman-Kluk step j: buffer KB[j & 1], complex.
+    constexpr int O_M2 = X::O_RP + (X::A_N - 2 * F) * G;
+    double Rr = 1.0, Ri = 0.0;
+    unsigned gk = 0u;
+    __syncwarp();  // every lane is done with the kept pivot columns
+    if (F > 1) {
+      const int own = act && l == 0;
+      const double r0 = rcp_nr2(W[0][F]);
+      sts_if(gsa + 8 * O_M2, r0, own);
+#pragma unroll
+      for (int i = F + 1; i < N; i++) sts_if(gsa + 8 * (O_M2 + (i - F) * G), W[0][i], own);
+      const double pr = Kr[0][0], pi = Ki[0][0];
+      const double rn = rcp_nr2(fma(pr, pr, pi * pi));
+      const uint32_t kb = gsa + 8 * X::O_KB;
+      sts_if(kb, pr * rn, own);
+      sts_if(kb + 8 * G, -pi * rn, own);
+#pragma unroll
+      for (int i = 1; i < F; i++) {
+        sts_if(kb + 8 * (2 * i) * G, Kr[0][i], own);
+        sts_if(kb + 8 * (2 * i + 1) * G, Ki[0][i], own);
+      }
       __syncwarp();
     }
 #pragma unroll
-    for (int k = F; k < N - 1; k++) {
-      const uint32_t b = gsa + 8 * (X::O_KB + ((k - F) & 1) * X::KBN * G);
-      const double r = lds(b);
+    for (int j = 0; j < F - 1; j++) {
+      const int k = F + j;
+      const uint32_t bm = gsa + 8 * (O_M2 + (j & 1) * F * G);
+      const uint32_t bk = gsa + 8 * (X::O_KB + (j & 1) * X::KBN * G);
+      const double r = lds(bm);
       double pc[N];
 #pragma unroll
-      for (int i = k + 1; i < N; i++) pc[i] = lds(b + 8 * (i - k) * G);
+      for (int i = k + 1; i < N; i++) pc[i] = lds(bm + 8 * (i - k) * G);
+      const double rr = lds(bk), ri = lds(bk + 8 * G);
+      double pr[F], pi[F];
+#pragma unroll
+      for (int i = j + 1; i < F; i++) {
+        pr[i] = lds(bk + 8 * (2 * (i - j)) * G);
+        pi[i] = lds(bk + 8 * (2 * (i - j) + 1) * G);
+      }
       Rm *= r;
-      const int sn = (k + 1 < N - 1) ? (k + 1 - F) / L : -1;
+      {
+        const double t = Rr * rr - Ri * ri;
+        Ri = fma(Rr, ri, Ri * rr);
+        Rr = t;
+      }
+      const int sn = (j + 1 < F - 1) ? (j + 1) / L : -1;  // the slot of the next pivot, in both eliminations
       if (sn >= 0) {
-        const double m = W[sn][k] * r;
-        if (F + sn * L + l > k && (X::EXACT || sn * L + l < F)) gm = max(gm, abs_hi(m));
+        const bool live = sn * L + l > j && (X::EXACT || sn * L + l < F);
+        const int own = act && l == (j + 1) % L;
+        {
+          const double m = W[sn][k] * r;
+          if (live) gm = max(gm, abs_hi(m));
 #pragma unroll
-        for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
-        const double rn = rcp_nr2(W[sn][k + 1]);
-        const int own = act && l == (k + 1 - F) % L;
-        const uint32_t nb = gsa + 8 * (X::O_KB + ((k + 1 - F) & 1) * X::KBN * G);
-        sts_if(nb, rn, own);
+          for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
+          const double rn = rcp_nr2(W[sn][k + 1]);
+          const uint32_t nb = gsa + 8 * (O_M2 + ((j + 1) & 1) * F * G);
+          sts_if(nb, rn, own);
 #pragma unroll
-        for (int i = k + 2; i < N; i++) sts_if(nb + 8 * (i - k - 1) * G, W[sn][i], own);
+          for (int i = k + 2; i < N; i++) sts_if(nb + 8 * (i - k - 1) * G, W[sn][i], own);
+        }
+        {
+          const double mr = Kr[sn][j] * rr - Ki[sn][j] * ri;
+          const double mi = fma(Kr[sn][j], ri, Ki[sn][j] * rr);
+          if (live) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+#pragma unroll
+          for (int i = j + 1; i < F; i++) {
+            Kr[sn][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[sn][i]));
+            Ki[sn][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[sn][i]));
+          }
+          const double qr = Kr[sn][j + 1], qi = Ki[sn][j + 1];
+          const double rn = rcp_nr2(fma(qr, qr, qi * qi));
+          const uint32_t nb = gsa + 8 * (X::O_KB + ((j + 1) & 1) * X::KBN * G);
+          sts_if(nb, qr * rn, own);
+          sts_if(nb + 8 * G, -qi * rn, own);
+#pragma unroll
+          for (int i = j + 2; i < F; i++) {
+            sts_if(nb + 8 * (2 * (i - j - 1)) * G, Kr[sn][i], own);
+            sts_if(nb + 8 * (2 * (i - j - 1) + 1) * G, Ki[sn][i], own);
+          }
+        }
         __syncwarp();
       }
 #pragma unroll
       for (int s = 0; s < C; s++) {
         if (s == sn) continue;
-        if (F + (s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= k) continue;
+        if ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= j) continue;  // dead on every lane
+        const bool live = s * L + l > j && (X::EXACT || s * L + l < F);
         const double m = W[s][k] * r;
-        if (F + s * L + l > k && (X::EXACT || s * L + l < F)) gm = max(gm, abs_hi(m));
+        if (live) gm = max(gm, abs_hi(m));
 #pragma unroll
         for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
+        const double mr = Kr[s][j] * rr - Ki[s][j] * ri;
+        const double mi = fma(Kr[s][j], ri, Ki[s][j] * rr);
+        if (live) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+#pragma unroll
+        for (int i = j + 1; i < F; i++) {
+          Kr[s][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[s][i]));
+          Ki[s][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[s][i]));
+        }
       }
     }
     detM = W[(F - 1) / L][N - 1] * rcp_nr2(Rm);
+    // det 2K = p_{F-1} / R  ~  p_{F-1} conj(R)
+    const double lr = Kr[(F - 1) / L][F - 1], li = Ki[(F - 1) / L][F - 1];
+    Dre = fma(lr, Rr, li * Ri);
+    Dim = fma(li, Rr, -lr * Ri);
+    gk_out = gk;
   }
   gm_out = gm;
 }
@@ -652,10 +733,9 @@ __device__ __forceinline__ void dets_cml(uint32_t tm, uint32_t gsa, int l, bool 
   dM = 1.0;
   gm = 0u;
   __syncwarp();  // region A changes hands: every lane is done with the Hessian slot of the pass
-  if (WITH_M) {
-    lu_m_cml<F, L>(tm, gsa, l, act, dM, gm);
-    __syncwarp();  // KB changes hands
-  }
+  if constexpr (WITH_M) {
+    lu_mk_cml<F, L>(tm, gsa, l, act, dM, gm, Dre, Dim, gk);
+  } else {
   double Kr[C][F], Ki[C][F];
 #pragma unroll
   for (int s = 0; s < C; s++) {
@@ -669,6 +749,7 @@ __device__ __forceinline__ void dets_cml(uint32_t tm, uint32_t gsa, int l, bool 
     }
   }
   lu_k_cml<F, L>(Kr, Ki, gsa, l, act, Dre, Dim, gk);
+  }
 }
 
 template <int F, int L, int KIND>
