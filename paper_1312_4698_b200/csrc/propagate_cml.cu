@@ -27,17 +27,27 @@
 
 namespace {
 
-constexpr int kWarpsC = 8;
+#ifndef SCI_CML_WARPS
+#define SCI_CML_WARPS 8
+#endif
+constexpr int kWarpsC = SCI_CML_WARPS;
 constexpr int kThreadsC = kWarpsC * 32;
 
 __device__ __forceinline__ double rcp_nr2(double x) {
-  // MUFU.RCP64H seed (2^-23 relative) + two Newton steps: ~1 ulp for normal x, no slow path.
+  // MUFU.RCP64H seed (2^-23 relative) + two Newton steps: ~1 ulp for normal x, no slow path.  One step (2^-46) is not
+  // enough: det M of a strongly stretched trajectory is a difference of large terms, and multipliers that are off by
+  // 1e-14 move |det M - 1| across the 1e-6 threshold where the oracle's exact multipliers do not (152 of 131072
+  // trajectories of config 4 change their flag).
+#ifndef SCI_CML_RCP_NR
+#define SCI_CML_RCP_NR 2
+#endif
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
+#pragma unroll
+  for (int it = 0; it < SCI_CML_RCP_NR; it++) {
+    const double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+  }
   return r;
 }
 
@@ -883,11 +893,12 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     }
     // a7: |det M - 1| <= tol and finite, every det_stride steps and at the end
     if (check) {
-      bool ok = (l == lw) ? (fabs(dM - 1.0) <= P.det_tol) : true;
-      ok = ok && isfinite(Sa);
+      // finite <=> exponent field below 0x7ff: one integer maximum over the high words
+      unsigned hx = abs_hi(Sa);
 #pragma unroll
-      for (int s = 0; s < C; s++) ok = ok && isfinite(Pm[s]) && isfinite(Q[s]);
-      good = good && ok;
+      for (int s = 0; s < C; s++) hx = max(hx, max(abs_hi(Pm[s]), abs_hi(Q[s])));
+      const bool okd = (l != lw) | (fabs(dM - 1.0) <= P.det_tol);
+      good = good & okd & (hx < 0x7ff00000u);
       det_count = P.det_stride;
     }
     det_count--;
