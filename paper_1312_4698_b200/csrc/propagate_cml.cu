@@ -60,22 +60,31 @@ __device__ __forceinline__ double lds(uint32_t a) {
   return v;
 }
 __device__ __forceinline__ void sts(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
-// predicated store: lanes with own == 0 issue nothing (no branch around the owner's publications)
-__device__ __forceinline__ void sts_if(uint32_t a, double v, int own) {
-  asm volatile("{ .reg .pred p; setp.ne.s32 p, %2, 0; @p st.shared.f64 [%0], %1; }" ::"r"(a), "d"(v), "r"(own) : "memory");
+__device__ __forceinline__ void lds2(uint32_t a, double &x, double &y) {
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(a) : "memory");
 }
+__device__ __forceinline__ void sts2(uint32_t a, double x, double y) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
+// value of v on lane src (every lane of the warp executes this).  One 64-bit broadcast costs two SHFL = one cycle of
+// the SM's shared-memory data pipe, against 2 (LDS.64) + 1.3 (owner's STS.64) + a warp barrier through shared memory
+// (ncu: l1tex__data_pipe_lsu_wavefronts_mem_shared, profiles/r02b)
+__device__ __forceinline__ double bcast(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
 template <int F, int L>
 struct Cml {
   static constexpr int C = (F + L - 1) / L;   // modes per lane
   static constexpr int G = 32 / L;            // trajectories per warp
-  static constexpr int ACT = G * L;           // lanes that own a trajectory share; the rest clone lane 0 and store nothing
+  static constexpr int ACT = G * L;           // lanes that own a trajectory share; the rest clone lane 0 (same numbers, same
+                                              // shared-memory stores) and write nothing to global memory
   static constexpr int N = 2 * F;             // rows of M: dP_0..dP_{F-1}, dQ_0..dQ_{F-1}
   static constexpr int NS = 2 * C;            // columns (slots) of M per lane
   static constexpr int ND = F / 2 + 1;        // Hessian entries (a, (a+d)%F), d = 0..ND-1, computed by the owner of mode a
   static constexpr int NR = (F - 1) / 2;      // cubic-gradient terms received from the owners of modes a-d
   static constexpr int NH = ND * F;
-  static constexpr int TCOLS = NS * N * 2;    // 32-bit TMEM columns per lane
+  // tensor memory, per lane, in doubles: [row half: dP rows, dQ rows][slot][F]
+  static constexpr int TH = NS * F;           // doubles per row half
+  static constexpr int TCOLS = 2 * TH * 2;    // 32-bit TMEM columns per lane
   static_assert(TCOLS <= 256, "state does not fit the half quadrant of tensor memory a warp owns");
   static constexpr bool EXACT = (F % L) == 0; // no phantom modes
   // packed coefficients.  QFF: per lane class l and slot s a list of LAP doubles, pair t of the list of (l, s) at
@@ -91,32 +100,59 @@ struct Cml {
   static constexpr int NCOEF = NCOEF_QFF > NCOEF_MORSE ? NCOEF_QFF : NCOEF_MORSE;
   static constexpr int NCOEFP = (NCOEF + 1) & ~1;
   // per-warp shared memory, in doubles.  Group arrays are [element][G] (the L lanes of trajectory g read the same word,
-  // the G trajectories adjacent words); the parked H dQ is lane-private, [element][32].
-  // Region A is used by the PES / pass phase (Q exchange, Hessian entries, cubic gradient terms) and, during the
-  // snapshot, by the pivot columns of the first F steps of the monodromy elimination, which are all kept (RP).
+  // the G trajectories adjacent words); the parked H dQ is lane-private, in pairs: element e of the lane at byte
+  // 512 (e / 2) + 16 lane + 8 (e % 2).
+  __host__ __device__ static constexpr int ev(int x) { return (x + 1) & ~1; }
   static constexpr int O_QS = 0;                      // [F]
-  static constexpr int O_HS = O_QS + F * G;           // [NH]
-  static constexpr int O_G3 = O_HS + NH * G;          // [NR][F]
-  static constexpr int PES_N = F + NH + NR * F;
-  static constexpr int RPN = F * N - F * (F - 1) / 2; // step k < F at offset rp(k): 1/pivot + rows k+1..N-1
-  static constexpr int O_RP = 0;
-  static constexpr int A_N = PES_N > RPN ? PES_N : RPN;
-  static constexpr int KBN = 2 * F;                   // doubles per buffer: complex 1/pivot + rows k+1..F-1 (a5), or the
-  static constexpr int O_KB = A_N * G;                // real 1/pivot + rows k+1..N-1 of a step k >= F (a7); [2][KBN]
-  static constexpr int O_RED = O_KB + 2 * KBN * G;    // [L][2]
-  static constexpr int O_HM = O_RED + 2 * L * G;      // [NS * F][32], lane-private
-  static constexpr int WS = O_HM + NS * F * 32;
+  static constexpr int O_HS = O_QS + F;               // [NH]
+  static constexpr int O_G3 = O_HS + NH;              // [NR][F]
+  static constexpr int O_RED = O_G3 + NR * F;         // [L][2]
+  static constexpr int O_DUMP = O_RED + 2 * L;        // [1]: stores of phantom modes (F % L != 0)
+  static constexpr int WSG = ev((O_DUMP + 1) * G);    // doubles of group arrays per warp
+  static constexpr int HMH = ev(C * F);               // parked H dQ: elements per half
+  static constexpr int WS = WSG + 2 * HMH * 32;
   static constexpr size_t SMEM = sizeof(double) * (NCOEFP + (size_t)kWarpsC * WS) + 16;
-  __host__ __device__ static constexpr int rp(int k) { return k * N - k * (k - 1) / 2; }
+  __host__ __device__ static constexpr int hm(int e) { return 512 * (e / 2) + 8 * (e % 2); }
 
   // column (l, s) of M: mode a = l + (s % C) L, half h = s / C (0: d/dP0_a, 1: d/dQ0_a), global index h F + a.
   // Elimination step k uses the diagonal pivot of the column with global index k.
   __host__ __device__ static constexpr int step_lane(int k) { return (k % F) % L; }
   __host__ __device__ static constexpr int step_slot(int k) { return (k % F) / L + (k / F) * C; }
-  // largest global index of slot s over the lane classes (is any lane's column s still live after step k?)
-  __host__ __device__ static constexpr int slot_max_index(int s) {
-    return (s / C) * F + (((s % C) * L + L - 1) < F - 1 ? ((s % C) * L + L - 1) : F - 1);
+  // is slot s (d/dP0 columns: s < C) still live on SOME lane class after the first k + 1 pivots?
+  __host__ __device__ static constexpr bool slot_live(int s, int k) {
+    return s >= C || ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) > k);
   }
+};
+
+// one column of M from / to the lane's tensor memory: rows 0..F-1 (dP) and F..2F-1 (dQ) live in different halves
+template <int F, int L>
+__device__ __forceinline__ void tmem_ld_col(uint32_t tm, int s, double (&col)[2 * F]) {
+  double a[F], b[F];
+  tmem_ld_f64<F>(tm + s * F * 2, a);
+  tmem_ld_f64<F>(tm + (Cml<F, L>::TH + s * F) * 2, b);
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    col[i] = a[i];
+    col[F + i] = b[i];
+  }
+}
+template <int F, int L>
+__device__ __forceinline__ void tmem_st_col(uint32_t tm, int s, const double (&col)[2 * F]) {
+  double a[F], b[F];
+#pragma unroll
+  for (int i = 0; i < F; i++) {
+    a[i] = col[i];
+    b[i] = col[F + i];
+  }
+  tmem_st_f64<F>(tm + s * F * 2, a);
+  tmem_st_f64<F>(tm + (Cml<F, L>::TH + s * F) * 2, b);
+}
+
+// shared-memory addresses of one lane
+struct LaneAddr {
+  uint32_t g;   // element 0 of the trajectory's group arrays: element e at g + 8 G e
+  uint32_t hm;  // the lane's parked H dQ
+  int g0;       // lane of class 0 of this trajectory: class c sits on lane g0 + c G
 };
 
 // ---- a1: potential share, gradient components and Hessian entries of the lane's modes (reduced coordinates) ----------
@@ -127,24 +163,26 @@ struct Cml {
 // Morse: y = exp(-a (Q - Q_e)), V = D (1-y)^2, g = 2 D a y (1-y), H = 2 D a^2 y (2y-1).
 // The owner of mode a computes the entries (a, (a+d)%F), d < ND, and stores them at HS[d F + a]; the cubic gradient
 // terms that belong to the modes a+d travel through G3.  Two warp barriers inside; the caller needs one more before
-// it reads HS.  gsa: shared address of the trajectory's group arrays (element e of array O at gsa + 8 (O + e G)).
+// it reads HS.  Stores of phantom modes (F % L != 0) go to the dump word.
 template <int F, int L, int KIND>
-__device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t gsa, int l, bool act,
-                                        const double (&Q)[Cml<F, L>::C], double (&gq)[Cml<F, L>::C], double &Va) {
+__device__ __forceinline__ void pes_cml(const double *__restrict__ cs, const LaneAddr &A, int l, const double (&Q)[Cml<F, L>::C],
+                                        double (&gq)[Cml<F, L>::C], double &Va) {
   using X = Cml<F, L>;
   constexpr int C = X::C, G = X::G;
+  const uint32_t gsa = A.g;
+  const uint32_t dump = gsa + 8 * X::O_DUMP * G;
   Va = 0.0;
   if (KIND == SC_IVR_PES_QFF) {
 #pragma unroll
     for (int s = 0; s < C; s++) {
       const int a = l + s * L;
-      sts_if(gsa + 8 * (X::O_QS + a * G), Q[s], act && (X::EXACT || a < F));
+      sts((X::EXACT || a < F) ? gsa + 8 * (X::O_QS + a) * G : dump, Q[s]);
     }
     __syncwarp();
     double q[F], q2[F];
 #pragma unroll
     for (int i = 0; i < F; i++) {
-      q[i] = lds(gsa + 8 * (X::O_QS + i * G));
+      q[i] = lds(gsa + 8 * (X::O_QS + i) * G);
       q2[i] = q[i] * q[i];
     }
     double s3[C], u[C], w2[C], paa[C];
@@ -154,7 +192,6 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t 
       const int a = l + s * L;
       const bool real = X::EXACT || a < F;
       const int ae = real ? a : 0;
-      const int own = act && real;
       double cf[X::LAP];
 #pragma unroll
       for (int t = 0; t < X::LAP / 2; t++) {
@@ -168,7 +205,7 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t 
       for (int d = 1; d < X::ND; d++) {
         int b = ae + d;
         b = b >= F ? b - F : b;
-        qd[d] = lds(gsa + 8 * (X::O_QS + b * G));
+        qd[d] = lds(gsa + 8 * (X::O_QS + b) * G);
       }
       double uu = 0.0;
 #pragma unroll
@@ -188,13 +225,13 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t 
       u[s] = uu;
       w2[s] = cf[X::L_W2];
       paa[s] = cf[X::L_C4D];
-      sts_if(gsa + 8 * (X::O_HS + ae * G), w2[s] + h3[0] + 0.5 * uu, own);
+      sts(real ? gsa + 8 * (X::O_HS + ae) * G : dump, w2[s] + h3[0] + 0.5 * uu);
 #pragma unroll
       for (int d = 1; d < X::ND; d++) {
         int b = ae + d;
         b = b >= F ? b - F : b;
-        sts_if(gsa + 8 * (X::O_HS + (d * F + ae) * G), fma(cf[X::L_C4D + d] * Q[s], qd[d], h3[d]), own);
-        if (d <= X::NR) sts_if(gsa + 8 * (X::O_G3 + ((d - 1) * F + b) * G), h3[d] * Q[s], own);
+        sts(real ? gsa + 8 * (X::O_HS + d * F + ae) * G : dump, fma(cf[X::L_C4D + d] * Q[s], qd[d], h3[d]));
+        if (d <= X::NR) sts(real ? gsa + 8 * (X::O_G3 + (d - 1) * F + b) * G : dump, h3[d] * Q[s]);
       }
     }
     __syncwarp();
@@ -205,7 +242,7 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t 
       const int ae = real ? a : 0;
       double t3 = s3[s];
 #pragma unroll
-      for (int d = 1; d <= X::NR; d++) t3 += lds(gsa + 8 * (X::O_G3 + ((d - 1) * F + ae) * G));
+      for (int d = 1; d <= X::NR; d++) t3 += lds(gsa + 8 * (X::O_G3 + (d - 1) * F + ae) * G);
       const double g3 = 0.5 * t3;
       const double g4 = Q[s] * (0.5 * u[s] - (1.0 / 3.0) * paa[s] * Q[s] * Q[s]);
       const double gg = fma(w2[s], Q[s], g3 + g4);
@@ -223,7 +260,7 @@ __device__ __forceinline__ void pes_cml(const double *__restrict__ cs, uint32_t 
       const double vv = D * (1.0 - y) * (1.0 - y);
       gq[s] = real ? 2.0 * D * at * y * (1.0 - y) : 0.0;
       Va += real ? vv : 0.0;
-      sts_if(gsa + 8 * (X::O_HS + (real ? a : 0) * G), 2.0 * D * at * at * y * (2.0 * y - 1.0), act && real);
+      sts(real ? gsa + 8 * (X::O_HS + a) * G : dump, 2.0 * D * at * at * y * (2.0 * y - 1.0));
     }
   }
 }
@@ -235,7 +272,7 @@ __device__ __forceinline__ void hessian_times(uint32_t gsa, const double (&dQ)[N
   constexpr int G = X::G;
 #pragma unroll
   for (int i = 0; i < F; i++) {
-    const double h = lds(gsa + 8 * (X::O_HS + i * G));
+    const double h = lds(gsa + 8 * (X::O_HS + i) * G);
 #pragma unroll
     for (int c = 0; c < NB; c++) HM[c][i] = h * dQ[c][i];
   }
@@ -246,7 +283,7 @@ __device__ __forceinline__ void hessian_times(uint32_t gsa, const double (&dQ)[N
       for (int i = 0; i < F; i++) {
         if (F % 2 == 0 && d == F / 2 && i >= F / 2) continue;  // pair (i, i+F/2) is also stored by the owner of i+F/2
         const int j = (i + d) % F;
-        const double h = lds(gsa + 8 * (X::O_HS + (d * F + i) * G));
+        const double h = lds(gsa + 8 * (X::O_HS + d * F + i) * G);
 #pragma unroll
         for (int c = 0; c < NB; c++) {
           HM[c][i] = fma(h, dQ[c][j], HM[c][i]);
@@ -260,336 +297,299 @@ __device__ __forceinline__ void hessian_times(uint32_t gsa, const double (&dQ)[N
 // ---- one pass over the lane's columns at a new evaluation point (a2, a3) ----------------------------------------------
 //   dP -= post * HMprev (opening kick of the point just left, H dQ parked there);  dQ += adt mu dP (drift);
 //   HM = H(Q_new) dQ;  dP -= pre * HM (kick at the new point up to the snapshot);  state -> TMEM;  HM parked.
-// Columns are handled C at a time (the slots of one half h).  hma: shared address of the lane's parked H dQ
-// (element e at hma + 256 e).
+// Columns are handled C at a time (the slots of one half h).
 template <int F, int L, int KIND>
-__device__ __forceinline__ void pass_cml(uint32_t tm, uint32_t gsa, uint32_t hma, const PropParams &P, double post,
-                                         double adt, double pre) {
+__device__ __forceinline__ void pass_cml(uint32_t tm, const LaneAddr &A, const PropParams &P, double post, double adt, double pre) {
   using X = Cml<F, L>;
-  constexpr int C = X::C, N = X::N;
+  constexpr int C = X::C;
 #pragma unroll
   for (int h = 0; h < 2; h++) {
-    double st[C * N];
-    tmem_ld_f64<C * N>(tm + h * C * N * 2, st);
+    double sp[C * F], sq[C * F];
+    tmem_ld_f64<C * F>(tm + h * C * F * 2, sp);
+    tmem_ld_f64<C * F>(tm + (X::TH + h * C * F) * 2, sq);
+    double hp[X::HMH];
+#pragma unroll
+    for (int e = 0; e < C * F; e += 2) lds2(A.hm + X::hm(h * X::HMH + e), hp[e], hp[e + 1]);
     double dP[C][F], dQ[C][F], HM[C][F];
 #pragma unroll
     for (int c = 0; c < C; c++)
 #pragma unroll
       for (int i = 0; i < F; i++) {
-        const double hp = lds(hma + 256 * ((h * C + c) * F + i));
-        dP[c][i] = fma(-post, hp, st[c * N + i]);
-        dQ[c][i] = fma(adt * P.mu[i], dP[c][i], st[c * N + F + i]);
+        dP[c][i] = fma(-post, hp[c * F + i], sp[c * F + i]);
+        dQ[c][i] = fma(adt * P.mu[i], dP[c][i], sq[c * F + i]);
       }
-    hessian_times<F, L, KIND, C>(gsa, dQ, HM);
+    hessian_times<F, L, KIND, C>(A.g, dQ, HM);
 #pragma unroll
     for (int c = 0; c < C; c++)
 #pragma unroll
       for (int i = 0; i < F; i++) {
-        st[c * N + i] = fma(-pre, HM[c][i], dP[c][i]);
-        st[c * N + F + i] = dQ[c][i];
-        sts(hma + 256 * ((h * C + c) * F + i), HM[c][i]);
+        sp[c * F + i] = fma(-pre, HM[c][i], dP[c][i]);
+        sq[c * F + i] = dQ[c][i];
       }
-    tmem_st_f64<C * N>(tm + h * C * N * 2, st);
+#pragma unroll
+    for (int e = 0; e < C * F; e += 2)
+      sts2(A.hm + X::hm(h * X::HMH + e), HM[e / F][e % F], (e + 1 < C * F) ? HM[(e + 1) / F][(e + 1) % F] : 0.0);
+    tmem_st_f64<C * F>(tm + h * C * F * 2, sp);
+    tmem_st_f64<C * F>(tm + (X::TH + h * C * F) * 2, sq);
   }
 }
 
-// ---- a7: det M by LU in a STATIC pivot order, in two column halves, with look-ahead ---------------------------------------
-// W[s][i]: row i of column s of the half in registers.  Step k eliminates row k with the diagonal pivot of the column
-// with global index k: its owner publishes (1/pivot, rows k+1..N-1 of the column) in the trajectory's shared slot,
-// every lane scales its row-k elements by the reciprocal and updates its live columns.  The column that holds the
-// NEXT pivot is updated first and published before the rest of the step's updates, so that the
-// reciprocal -> store -> barrier -> load chain of step k+1 runs under the bulk of step k's arithmetic.
-// Halves: steps 0..F-1 (pivots in the d/dP0 columns) touch only the d/dP0 columns while their pivot columns are all
-// KEPT in shared memory (region RP); then the d/dQ0 columns are loaded, catch up on those F steps without any
-// barrier, and steps F..N-2 run among them (buffers in KB).  Same arithmetic as the one-piece elimination, half the
-// registers.  No pivot search: numerical safety is monitored instead (gm = largest |multiplier| of a live column,
-// IEEE high word); the caller repeats a step whose multipliers exceed its bound with the pivoted routine.
-// Result on lane step_lane(N-1): det M.
+// ---- a5: the F-1 steps of the complex elimination of 2K, one at a time (called from both snapshot variants) -------------
+// (rr, ri): reciprocal pivot of step j; (pr, pi)[i], i > j: the pivot column.  sn: slot that holds the next pivot (-1:
+// none); on return (nr, ni)[i], i >= j + 1 hold the next pivot column as broadcast by its owner, row j + 1 the pivot.
 template <int F, int L>
-__device__ __forceinline__ void lu_mk_cml(uint32_t tm, uint32_t gsa, int l, bool act, double &detM, unsigned &gm_out,
-                                          double &Dre, double &Dim, unsigned &gk_out) {
+struct KStep {
   using X = Cml<F, L>;
-  constexpr int G = X::G, N = X::N, C = X::C;
+  static constexpr int C = X::C, G = X::G;
+  // update slot s with step j
+  static __device__ __forceinline__ void upd(int j, int s, int l, double (&Kr)[C][F], double (&Ki)[C][F], double rr, double ri,
+                                             const double (&pr)[F], const double (&pi)[F], unsigned &gk) {
+    const bool live = s * L + l > j && (X::EXACT || s * L + l < F);
+    const double mr = Kr[s][j] * rr - Ki[s][j] * ri;
+    const double mi = fma(Kr[s][j], ri, Ki[s][j] * rr);
+    if (live) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+#pragma unroll
+    for (int i = j + 1; i < F; i++) {
+      Kr[s][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[s][i]));
+      Ki[s][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[s][i]));
+    }
+  }
+  // broadcast column `s` (rows j..F-1) from lane class c; row j is replaced by the reciprocal of the pivot
+  static __device__ __forceinline__ void cast(int j, int s, int src, const double (&Kr)[C][F], const double (&Ki)[C][F], double &rr,
+                                              double &ri, double (&pr)[F], double (&pi)[F]) {
+#pragma unroll
+    for (int i = j; i < F; i++) {
+      pr[i] = bcast(Kr[s][i], src);
+      pi[i] = bcast(Ki[s][i], src);
+    }
+    const double rn = rcp_nr2(fma(pr[j], pr[j], pi[j] * pi[j]));
+    rr = pr[j] * rn;
+    ri = -pi[j] * rn;
+  }
+};
+
+// ---- a7 + a5: det M by LU in a STATIC pivot order with look-ahead, in two ROW halves; det 2K alongside --------------------
+// The lane holds NS = 2C columns of M (slot s < C: d/dP0 of its mode s, slot C + s: d/dQ0).  Step k eliminates row k with
+// the diagonal pivot of the column with global index k: every lane receives that column from its owner by warp shuffles
+// (no shared memory, no barrier), scales its row-k elements by the reciprocal pivot (multiplier m[s][k]) and updates its
+// live columns.  The column that holds the NEXT pivot is updated first and broadcast before the rest of the step's
+// updates, so that the shuffle -> reciprocal chain of step k+1 runs under the bulk of step k's arithmetic.
+// Row halves (the registers hold 2C x F doubles of M at a time): phase T runs the steps 0..F-1 on the rows 0..F-1 (dP) of all
+// columns and keeps the multipliers; phase B replays them on the rows F..2F-1 (dQ), the pivot columns' lower parts being
+// broadcast as they become final; what is left in the d/dQ0 columns is the Schur complement, whose F-1 steps run TOGETHER
+// with the F-1 steps of the complex elimination of 2K (two independent pivot chains).  Element by element the arithmetic
+// is that of the one-piece right-looking elimination.  No pivot search: numerical safety is monitored instead (gm, gk =
+// largest |multiplier| of a live column, IEEE high word); the caller repeats a step whose multipliers exceed its bound
+// with the pivoted routine.
+// Results on lane class step_lane(N-1): det M, and (Dre, Dim) = det(2K) |R|^2 with R the product of the reciprocal
+// pivots: a positive multiple of det 2K; only its phase is used downstream (Eq. 10 drops |C_t|).
+template <int F, int L>
+__device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l, double &detM, unsigned &gm_out, double &Dre,
+                                          double &Dim, unsigned &gk_out) {
+  using X = Cml<F, L>;
+  constexpr int G = X::G, C = X::C, NS = X::NS;
   double Rm = 1.0;
   unsigned gm = 0u;
+  double m[NS][F];  // m[s][k]: multiplier of column s in step k (entries of dead columns are never used)
+  // ---- phase T: rows 0..F-1 ----
   {
-    double W[C][N];
+    double W[NS][F];
     {
-      double st[C * N];
-      tmem_ld_f64<C * N>(tm, st);
+      double st[NS * F];
+      tmem_ld_f64<NS * F>(tm, st);
 #pragma unroll
-      for (int s = 0; s < C; s++)
+      for (int s = 0; s < NS; s++)
 #pragma unroll
-        for (int i = 0; i < N; i++) W[s][i] = st[s * N + i];
+        for (int i = 0; i < F; i++) W[s][i] = st[s * F + i];
     }
-    {
-      const double r0 = rcp_nr2(W[0][0]);
-      const int own = act && l == 0;
-      sts_if(gsa + 8 * (X::O_RP + 0), r0, own);
+    double pc[F];
 #pragma unroll
-      for (int i = 1; i < N; i++) sts_if(gsa + 8 * (X::O_RP + i * G), W[0][i], own);
-    }
-    __syncwarp();
+    for (int i = 0; i < F; i++) pc[i] = bcast(W[0][i], A.g0);
+    double r = rcp_nr2(pc[0]);
 #pragma unroll
     for (int k = 0; k < F; k++) {
-      const uint32_t b = gsa + 8 * (X::O_RP + X::rp(k) * G);
-      const double r = lds(b);
-      double pc[N];
-#pragma unroll
-      for (int i = k + 1; i < N; i++) pc[i] = lds(b + 8 * (i - k) * G);
       Rm *= r;
       const int sn = (k + 1 < F) ? (k + 1) / L : -1;
+      double pn[F], rn = 0.0;
       if (sn >= 0) {
-        const double m = W[sn][k] * r;
-        if (sn * L + l > k && (X::EXACT || sn * L + l < F)) gm = max(gm, abs_hi(m));
+        m[sn][k] = W[sn][k] * r;
+        if (sn * L + l > k && (X::EXACT || sn * L + l < F)) gm = max(gm, abs_hi(m[sn][k]));
 #pragma unroll
-        for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
-        const double rn = rcp_nr2(W[sn][k + 1]);
-        const int own = act && l == (k + 1) % L;
-        const uint32_t nb = gsa + 8 * (X::O_RP + X::rp(k + 1) * G);
-        sts_if(nb, rn, own);
+        for (int i = k + 1; i < F; i++) W[sn][i] = fma(-m[sn][k], pc[i], W[sn][i]);
 #pragma unroll
-        for (int i = k + 2; i < N; i++) sts_if(nb + 8 * (i - k - 1) * G, W[sn][i], own);
-        __syncwarp();
+        for (int i = k + 1; i < F; i++) pn[i] = bcast(W[sn][i], A.g0 + ((k + 1) % L) * G);
+        rn = rcp_nr2(pn[k + 1]);
       }
 #pragma unroll
-      for (int s = 0; s < C; s++) {
-        if (s == sn) continue;
-        if ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= k) continue;  // dead on every lane
-        const double m = W[s][k] * r;
-        if (s * L + l > k && (X::EXACT || s * L + l < F)) gm = max(gm, abs_hi(m));
+      for (int s = 0; s < NS; s++) {
+        if (s == sn || !X::slot_live(s, k)) continue;
+        m[s][k] = W[s][k] * r;
+        const bool live = s >= C ? (X::EXACT || (s - C) * L + l < F) : (s * L + l > k && (X::EXACT || s * L + l < F));
+        if (live) gm = max(gm, abs_hi(m[s][k]));
 #pragma unroll
-        for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
+        for (int i = k + 1; i < F; i++) W[s][i] = fma(-m[s][k], pc[i], W[s][i]);
+      }
+      if (sn >= 0) {
+        r = rn;
+#pragma unroll
+        for (int i = k + 2; i < F; i++) pc[i] = pn[i];
       }
     }
+  }
+  // ---- phase B: rows F..2F-1 (W[s][i] is row F + i) ----
+  double W[NS][F];
+  {
+    double st[NS * F];
+    tmem_ld_f64<NS * F>(tm + X::TH * 2, st);
+#pragma unroll
+    for (int s = 0; s < NS; s++)
+#pragma unroll
+      for (int i = 0; i < F; i++) W[s][i] = st[s * F + i];
   }
   {
-    double W[C][N];  // the d/dQ0 columns: global index F + s L + l
-    {
-      double st[C * N];
-      tmem_ld_f64<C * N>(tm + C * N * 2, st);
+    double pc[F];
 #pragma unroll
-      for (int s = 0; s < C; s++)
-#pragma unroll
-        for (int i = 0; i < N; i++) W[s][i] = st[s * N + i];
-    }
-    // catch up on steps 0..F-1 (every column of this half is live during them)
+    for (int i = 0; i < F; i++) pc[i] = bcast(W[0][i], A.g0);
 #pragma unroll
     for (int k = 0; k < F; k++) {
-      const uint32_t b = gsa + 8 * (X::O_RP + X::rp(k) * G);
-      const double r = lds(b);
-      double m[C];
-#pragma unroll
-      for (int s = 0; s < C; s++) {
-        m[s] = W[s][k] * r;
-        if (X::EXACT || s * L + l < F) gm = max(gm, abs_hi(m[s]));
-      }
-#pragma unroll
-      for (int i = k + 1; i < N; i++) {
-        const double x = lds(b + 8 * (i - k) * G);
-#pragma unroll
-        for (int s = 0; s < C; s++) W[s][i] = fma(-m[s], x, W[s][i]);
-      }
-    }
-    // the lane's columns of 2K = (M_qq + M_pp) + i (M_pq - M_qp) (Eq. 5, reading R2, reduced coordinates)
-    double Kr[C][F], Ki[C][F];
-#pragma unroll
-    for (int s = 0; s < C; s++) {
-      double c1[N], c2[N];  // columns d/dP0_a and d/dQ0_a of the lane's mode s
-      tmem_ld_f64<N>(tm + s * N * 2, c1);
-      tmem_ld_f64<N>(tm + (C + s) * N * 2, c2);
-#pragma unroll
-      for (int i = 0; i < F; i++) {
-        Kr[s][i] = c2[F + i] + c1[i];  // dQ2 + dP1
-        Ki[s][i] = c2[i] - c1[F + i];  // dP2 - dQ1
-      }
-    }
-    // steps F..N-2 among the d/dQ0 columns run TOGETHER with the F-1 steps of the complex elimination of 2K: two
-    // independent pivot chains per barrier.  Monodromy step k = F + j: buffer M2[j & 1] (the tail of region A, free once
-    // every lane has caught up), 1/pivot + rows k+1..N-1; Herman-Kluk step j: buffer KB[j & 1], complex.
-    constexpr int O_M2 = X::O_RP + (X::A_N - 2 * F) * G;
-    double Rr = 1.0, Ri = 0.0;
-    unsigned gk = 0u;
-    __syncwarp();  // every lane is done with the kept pivot columns
-    if (F > 1) {
-      const int own = act && l == 0;
-      const double r0 = rcp_nr2(W[0][F]);
-      sts_if(gsa + 8 * O_M2, r0, own);
-#pragma unroll
-      for (int i = F + 1; i < N; i++) sts_if(gsa + 8 * (O_M2 + (i - F) * G), W[0][i], own);
-      const double pr = Kr[0][0], pi = Ki[0][0];
-      const double rn = rcp_nr2(fma(pr, pr, pi * pi));
-      const uint32_t kb = gsa + 8 * X::O_KB;
-      sts_if(kb, pr * rn, own);
-      sts_if(kb + 8 * G, -pi * rn, own);
-#pragma unroll
-      for (int i = 1; i < F; i++) {
-        sts_if(kb + 8 * (2 * i) * G, Kr[0][i], own);
-        sts_if(kb + 8 * (2 * i + 1) * G, Ki[0][i], own);
-      }
-      __syncwarp();
-    }
-#pragma unroll
-    for (int j = 0; j < F - 1; j++) {
-      const int k = F + j;
-      const uint32_t bm = gsa + 8 * (O_M2 + (j & 1) * F * G);
-      const uint32_t bk = gsa + 8 * (X::O_KB + (j & 1) * X::KBN * G);
-      const double r = lds(bm);
-      double pc[N];
-#pragma unroll
-      for (int i = k + 1; i < N; i++) pc[i] = lds(bm + 8 * (i - k) * G);
-      const double rr = lds(bk), ri = lds(bk + 8 * G);
-      double pr[F], pi[F];
-#pragma unroll
-      for (int i = j + 1; i < F; i++) {
-        pr[i] = lds(bk + 8 * (2 * (i - j)) * G);
-        pi[i] = lds(bk + 8 * (2 * (i - j) + 1) * G);
-      }
-      Rm *= r;
-      {
-        const double t = Rr * rr - Ri * ri;
-        Ri = fma(Rr, ri, Ri * rr);
-        Rr = t;
-      }
-      const int sn = (j + 1 < F - 1) ? (j + 1) / L : -1;  // the slot of the next pivot, in both eliminations
+      const int sn = (k + 1 < F) ? (k + 1) / L : -1;
+      double pn[F];
       if (sn >= 0) {
-        const bool live = sn * L + l > j && (X::EXACT || sn * L + l < F);
-        const int own = act && l == (j + 1) % L;
-        {
-          const double m = W[sn][k] * r;
-          if (live) gm = max(gm, abs_hi(m));
 #pragma unroll
-          for (int i = k + 1; i < N; i++) W[sn][i] = fma(-m, pc[i], W[sn][i]);
-          const double rn = rcp_nr2(W[sn][k + 1]);
-          const uint32_t nb = gsa + 8 * (O_M2 + ((j + 1) & 1) * F * G);
-          sts_if(nb, rn, own);
+        for (int i = 0; i < F; i++) W[sn][i] = fma(-m[sn][k], pc[i], W[sn][i]);
 #pragma unroll
-          for (int i = k + 2; i < N; i++) sts_if(nb + 8 * (i - k - 1) * G, W[sn][i], own);
-        }
-        {
-          const double mr = Kr[sn][j] * rr - Ki[sn][j] * ri;
-          const double mi = fma(Kr[sn][j], ri, Ki[sn][j] * rr);
-          if (live) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
-#pragma unroll
-          for (int i = j + 1; i < F; i++) {
-            Kr[sn][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[sn][i]));
-            Ki[sn][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[sn][i]));
-          }
-          const double qr = Kr[sn][j + 1], qi = Ki[sn][j + 1];
-          const double rn = rcp_nr2(fma(qr, qr, qi * qi));
-          const uint32_t nb = gsa + 8 * (X::O_KB + ((j + 1) & 1) * X::KBN * G);
-          sts_if(nb, qr * rn, own);
-          sts_if(nb + 8 * G, -qi * rn, own);
-#pragma unroll
-          for (int i = j + 2; i < F; i++) {
-            sts_if(nb + 8 * (2 * (i - j - 1)) * G, Kr[sn][i], own);
-            sts_if(nb + 8 * (2 * (i - j - 1) + 1) * G, Ki[sn][i], own);
-          }
-        }
-        __syncwarp();
+        for (int i = 0; i < F; i++) pn[i] = bcast(W[sn][i], A.g0 + ((k + 1) % L) * G);
       }
 #pragma unroll
-      for (int s = 0; s < C; s++) {
-        if (s == sn) continue;
-        if ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= j) continue;  // dead on every lane
-        const bool live = s * L + l > j && (X::EXACT || s * L + l < F);
-        const double m = W[s][k] * r;
-        if (live) gm = max(gm, abs_hi(m));
+      for (int s = 0; s < NS; s++) {
+        if (s == sn || !X::slot_live(s, k)) continue;
 #pragma unroll
-        for (int i = k + 1; i < N; i++) W[s][i] = fma(-m, pc[i], W[s][i]);
-        const double mr = Kr[s][j] * rr - Ki[s][j] * ri;
-        const double mi = fma(Kr[s][j], ri, Ki[s][j] * rr);
-        if (live) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+        for (int i = 0; i < F; i++) W[s][i] = fma(-m[s][k], pc[i], W[s][i]);
+      }
+      if (sn >= 0) {
 #pragma unroll
-        for (int i = j + 1; i < F; i++) {
-          Kr[s][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[s][i]));
-          Ki[s][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[s][i]));
-        }
+        for (int i = 0; i < F; i++) pc[i] = pn[i];
       }
     }
-    detM = W[(F - 1) / L][N - 1] * rcp_nr2(Rm);
-    // det 2K = p_{F-1} / R  ~  p_{F-1} conj(R)
-    const double lr = Kr[(F - 1) / L][F - 1], li = Ki[(F - 1) / L][F - 1];
-    Dre = fma(lr, Rr, li * Ri);
-    Dim = fma(li, Rr, -lr * Ri);
-    gk_out = gk;
   }
-  gm_out = gm;
-}
-
-// ---- a5: det 2K (complex F x F; the lane's columns s = 0..C-1 are those of its modes) by the same scheme ------------------
-// Result on lane step_lane(F-1): (Dre, Dim) = det(2K) |R|^2 with R the product of the reciprocal pivots: a positive
-// multiple of det 2K; only its phase is used downstream (Eq. 10 drops |C_t|).
-template <int F, int L>
-__device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (&Ki)[Cml<F, L>::C][F], uint32_t gsa, int l,
-                                         bool act, double &Dre, double &Dim, unsigned &gk_out) {
-  using X = Cml<F, L>;
-  constexpr int G = X::G, C = X::C;
+  // ---- the Schur complement S[s][i] = W[C + s][i] (F x F, column index s L + l) and 2K ----
+  // the lane's columns of 2K = (M_qq + M_pp) + i (M_pq - M_qp) (Eq. 5, reading R2, reduced coordinates)
+  double Kr[C][F], Ki[C][F];
+#pragma unroll
+  for (int s = 0; s < C; s++) {
+    double c1p[F], c1q[F], c2p[F], c2q[F];  // columns d/dP0_a and d/dQ0_a of the lane's mode s, dP rows and dQ rows
+    tmem_ld_f64<F>(tm + s * F * 2, c1p);
+    tmem_ld_f64<F>(tm + (X::TH + s * F) * 2, c1q);
+    tmem_ld_f64<F>(tm + (C + s) * F * 2, c2p);
+    tmem_ld_f64<F>(tm + (X::TH + (C + s) * F) * 2, c2q);
+#pragma unroll
+    for (int i = 0; i < F; i++) {
+      Kr[s][i] = c2q[i] + c1p[i];  // dQ2 + dP1
+      Ki[s][i] = c2p[i] - c1q[i];  // dP2 - dQ1
+    }
+  }
   double Rr = 1.0, Ri = 0.0;
   unsigned gk = 0u;
+  double pc[F], r = 1.0;
+  double rr = 1.0, ri = 0.0, pr[F], pi[F];
   if (F > 1) {
-    const double pr = Kr[0][0], pi = Ki[0][0];
-    const double rn = rcp_nr2(fma(pr, pr, pi * pi));
-    const int own = act && l == 0;
-    const uint32_t b = gsa + 8 * X::O_KB;
-    sts_if(b, pr * rn, own);
-    sts_if(b + 8 * G, -pi * rn, own);
 #pragma unroll
-    for (int i = 1; i < F; i++) {
-      sts_if(b + 8 * (2 * i) * G, Kr[0][i], own);
-      sts_if(b + 8 * (2 * i + 1) * G, Ki[0][i], own);
-    }
-    __syncwarp();
+    for (int i = 0; i < F; i++) pc[i] = bcast(W[C][i], A.g0);
+    r = rcp_nr2(pc[0]);
+    KStep<F, L>::cast(0, 0, A.g0, Kr, Ki, rr, ri, pr, pi);
   }
 #pragma unroll
-  for (int k = 0; k < F - 1; k++) {
-    const uint32_t b = gsa + 8 * (X::O_KB + (k & 1) * X::KBN * G);
-    const double rr = lds(b), ri = lds(b + 8 * G);
-    double pr[F], pi[F];
-#pragma unroll
-    for (int i = k + 1; i < F; i++) {
-      pr[i] = lds(b + 8 * (2 * (i - k)) * G);
-      pi[i] = lds(b + 8 * (2 * (i - k) + 1) * G);
-    }
+  for (int j = 0; j < F - 1; j++) {
+    Rm *= r;
     {
       const double t = Rr * rr - Ri * ri;
       Ri = fma(Rr, ri, Ri * rr);
       Rr = t;
     }
-    const int sn = (k + 1 < F - 1) ? (k + 1) / L : -1;
+    const int sn = (j + 1 < F - 1) ? (j + 1) / L : -1;  // the slot of the next pivot, in both eliminations
+    double pn[F], rn = 0.0, rrn = 0.0, rin = 0.0, prn[F], pin[F];
     if (sn >= 0) {
-      const double mr = Kr[sn][k] * rr - Ki[sn][k] * ri;
-      const double mi = fma(Kr[sn][k], ri, Ki[sn][k] * rr);
-      if (sn * L + l > k && (X::EXACT || sn * L + l < F)) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+      const bool live = sn * L + l > j && (X::EXACT || sn * L + l < F);
+      const int src = A.g0 + ((j + 1) % L) * G;
+      {
+        const double mm = W[C + sn][j] * r;
+        if (live) gm = max(gm, abs_hi(mm));
 #pragma unroll
-      for (int i = k + 1; i < F; i++) {
-        Kr[sn][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[sn][i]));
-        Ki[sn][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[sn][i]));
-      }
-      const double qr = Kr[sn][k + 1], qi = Ki[sn][k + 1];
-      const double rn = rcp_nr2(fma(qr, qr, qi * qi));
-      const int own = act && l == (k + 1) % L;
-      const uint32_t nb = gsa + 8 * (X::O_KB + ((k + 1) & 1) * X::KBN * G);
-      sts_if(nb, qr * rn, own);
-      sts_if(nb + 8 * G, -qi * rn, own);
+        for (int i = j + 1; i < F; i++) W[C + sn][i] = fma(-mm, pc[i], W[C + sn][i]);
 #pragma unroll
-      for (int i = k + 2; i < F; i++) {
-        sts_if(nb + 8 * (2 * (i - k - 1)) * G, Kr[sn][i], own);
-        sts_if(nb + 8 * (2 * (i - k - 1) + 1) * G, Ki[sn][i], own);
+        for (int i = j + 1; i < F; i++) pn[i] = bcast(W[C + sn][i], src);
+        rn = rcp_nr2(pn[j + 1]);
       }
-      __syncwarp();
+      KStep<F, L>::upd(j, sn, l, Kr, Ki, rr, ri, pr, pi, gk);
+      KStep<F, L>::cast(j + 1, sn, src, Kr, Ki, rrn, rin, prn, pin);
     }
 #pragma unroll
     for (int s = 0; s < C; s++) {
-      if (s == sn) continue;
-      if ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) <= k) continue;
-      const double mr = Kr[s][k] * rr - Ki[s][k] * ri;
-      const double mi = fma(Kr[s][k], ri, Ki[s][k] * rr);
-      if (s * L + l > k && (X::EXACT || s * L + l < F)) gk = max(gk, max(abs_hi(mr), abs_hi(mi)));
+      if (s == sn || !X::slot_live(s, j)) continue;
+      const bool live = s * L + l > j && (X::EXACT || s * L + l < F);
+      const double mm = W[C + s][j] * r;
+      if (live) gm = max(gm, abs_hi(mm));
 #pragma unroll
-      for (int i = k + 1; i < F; i++) {
-        Kr[s][i] = fma(-mr, pr[i], fma(mi, pi[i], Kr[s][i]));
-        Ki[s][i] = fma(-mr, pi[i], fma(-mi, pr[i], Ki[s][i]));
+      for (int i = j + 1; i < F; i++) W[C + s][i] = fma(-mm, pc[i], W[C + s][i]);
+      KStep<F, L>::upd(j, s, l, Kr, Ki, rr, ri, pr, pi, gk);
+    }
+    if (sn >= 0) {
+      r = rn;
+      rr = rrn;
+      ri = rin;
+#pragma unroll
+      for (int i = j + 2; i < F; i++) {
+        pc[i] = pn[i];
+        pr[i] = prn[i];
+        pi[i] = pin[i];
+      }
+    }
+  }
+  detM = W[C + (F - 1) / L][F - 1] * rcp_nr2(Rm);
+  // det 2K = p_{F-1} / R  ~  p_{F-1} conj(R)
+  const double lr = Kr[(F - 1) / L][F - 1], li = Ki[(F - 1) / L][F - 1];
+  Dre = fma(lr, Rr, li * Ri);
+  Dim = fma(li, Rr, -lr * Ri);
+  gk_out = gk;
+  gm_out = gm;
+}
+
+// ---- a5 alone (time steps without the a7 check): det 2K by the same scheme; the lane's columns s = 0..C-1 are those of
+// its modes.  Result on lane class step_lane(F-1).
+template <int F, int L>
+__device__ __forceinline__ void lu_k_cml(double (&Kr)[Cml<F, L>::C][F], double (&Ki)[Cml<F, L>::C][F], const LaneAddr &A, int l,
+                                         double &Dre, double &Dim, unsigned &gk_out) {
+  using X = Cml<F, L>;
+  constexpr int G = X::G, C = X::C;
+  double Rr = 1.0, Ri = 0.0;
+  unsigned gk = 0u;
+  double rr = 1.0, ri = 0.0, pr[F], pi[F];
+  if (F > 1) KStep<F, L>::cast(0, 0, A.g0, Kr, Ki, rr, ri, pr, pi);
+#pragma unroll
+  for (int j = 0; j < F - 1; j++) {
+    {
+      const double t = Rr * rr - Ri * ri;
+      Ri = fma(Rr, ri, Ri * rr);
+      Rr = t;
+    }
+    const int sn = (j + 1 < F - 1) ? (j + 1) / L : -1;
+    double rrn = 0.0, rin = 0.0, prn[F], pin[F];
+    if (sn >= 0) {
+      KStep<F, L>::upd(j, sn, l, Kr, Ki, rr, ri, pr, pi, gk);
+      KStep<F, L>::cast(j + 1, sn, A.g0 + ((j + 1) % L) * G, Kr, Ki, rrn, rin, prn, pin);
+    }
+#pragma unroll
+    for (int s = 0; s < C; s++) {
+      if (s == sn || !X::slot_live(s, j)) continue;
+      KStep<F, L>::upd(j, s, l, Kr, Ki, rr, ri, pr, pi, gk);
+    }
+    if (sn >= 0) {
+      rr = rrn;
+      ri = rin;
+#pragma unroll
+      for (int i = j + 2; i < F; i++) {
+        pr[i] = prn[i];
+        pi[i] = pin[i];
       }
     }
   }
@@ -613,7 +613,7 @@ __device__ __noinline__ void pivoted_dets_cml(uint32_t tm, int g, bool with_m, d
 #pragma unroll
   for (int s = 0; s < NS; s++) {
     double col[N];
-    tmem_ld_f64<N>(tm + s * N * 2, col);
+    tmem_ld_col<F, L>(tm, s, col);
 #pragma unroll
     for (int lp = 0; lp < L; lp++) {
       const int a = lp + (s % C) * L;
@@ -736,29 +736,28 @@ __device__ __noinline__ void pivoted_dets_cml(uint32_t tm, int g, bool with_m, d
 
 // ---- snapshot: both determinants of M(c) from the TMEM state -----------------------------------------------------------
 template <int F, int L, bool WITH_M>
-__device__ __forceinline__ void dets_cml(uint32_t tm, uint32_t gsa, int l, bool act, double &Dre, double &Dim, double &dM,
+__device__ __forceinline__ void dets_cml(uint32_t tm, const LaneAddr &A, int l, double &Dre, double &Dim, double &dM,
                                          unsigned &gk, unsigned &gm) {
   using X = Cml<F, L>;
   constexpr int C = X::C, N = X::N;
   dM = 1.0;
   gm = 0u;
-  __syncwarp();  // region A changes hands: every lane is done with the Hessian slot of the pass
   if constexpr (WITH_M) {
-    lu_mk_cml<F, L>(tm, gsa, l, act, dM, gm, Dre, Dim, gk);
+    lu_mk_cml<F, L>(tm, A, l, dM, gm, Dre, Dim, gk);
   } else {
   double Kr[C][F], Ki[C][F];
 #pragma unroll
   for (int s = 0; s < C; s++) {
     double c1[N], c2[N];  // columns d/dP0_a and d/dQ0_a of the lane's mode s
-    tmem_ld_f64<N>(tm + s * N * 2, c1);
-    tmem_ld_f64<N>(tm + (C + s) * N * 2, c2);
+    tmem_ld_col<F, L>(tm, s, c1);
+    tmem_ld_col<F, L>(tm, C + s, c2);
 #pragma unroll
     for (int i = 0; i < F; i++) {
       Kr[s][i] = c2[F + i] + c1[i];  // dQ2 + dP1
       Ki[s][i] = c2[i] - c1[F + i];  // dP2 - dQ1
     }
   }
-  lu_k_cml<F, L>(Kr, Ki, gsa, l, act, Dre, Dim, gk);
+  lu_k_cml<F, L>(Kr, Ki, A, l, Dre, Dim, gk);
   }
 }
 
@@ -785,8 +784,10 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
   const bool act = lane < X::ACT;
   const int l = act ? lane / G : 0, g = act ? lane - l * G : 0;
   double *ws = smem + X::NCOEFP + warp * X::WS;
-  const uint32_t gsa = (uint32_t)__cvta_generic_to_shared(ws + g);                // group arrays
-  const uint32_t hma = (uint32_t)__cvta_generic_to_shared(ws + X::O_HM + lane);   // parked H dQ
+  LaneAddr A;
+  A.g = (uint32_t)__cvta_generic_to_shared(ws + g);
+  A.hm = (uint32_t)__cvta_generic_to_shared(ws + X::WSG) + 16 * lane;
+  A.g0 = g;
   unsigned gmask = 0u;
 #pragma unroll
   for (int i = 0; i < L; i++) gmask |= 1u << (i * G + g);
@@ -817,13 +818,13 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     const int a = l + (s % C) * L;
 #pragma unroll
     for (int i = 0; i < N; i++) col[i] = (i == (s / C) * F + a && (X::EXACT || a < F)) ? 1.0 : 0.0;
-    tmem_st_f64<N>(tm + s * N * 2, col);
+    tmem_st_col<F, L>(tm, s, col);
   }
 #pragma unroll 1
-  for (int e = 0; e < NS * F; e++) sts(hma + 256 * e, 0.0);
-  pes_cml<F, L, KIND>(cs, gsa, l, act, Q, gq, Va);
+  for (int e = 0; e < X::HMH; e++) sts2(A.hm + 512 * e, 0.0, 0.0);
+  pes_cml<F, L, KIND>(cs, A, l, Q, gq, Va);
   __syncwarp();
-  pass_cml<F, L, KIND>(tm, gsa, hma, P, 0.0, 0.0, 0.0);
+  pass_cml<F, L, KIND>(tm, A, P, 0.0, 0.0, 0.0);
 
   const int lw = X::step_lane(N - 1);  // the lane class that ends up with the last pivots of both eliminations
   bool good = true;
@@ -849,13 +850,13 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         oa = 0.0;
         ob = Sa;
       }
-      sts_if(gsa + 8 * (X::O_RED + (2 * l) * G), oa, act);
-      sts_if(gsa + 8 * (X::O_RED + (2 * l + 1) * G), ob, act);
+      sts(A.g + 8 * (X::O_RED + 2 * l) * G, oa);
+      sts(A.g + 8 * (X::O_RED + 2 * l + 1) * G, ob);
     }
     double Dre, Dim, dM;
     unsigned growK, growM;
-    if (check) dets_cml<F, L, true>(tm, gsa, l, act, Dre, Dim, dM, growK, growM);
-    else dets_cml<F, L, false>(tm, gsa, l, act, Dre, Dim, dM, growK, growM);
+    if (check) dets_cml<F, L, true>(tm, A, l, Dre, Dim, dM, growK, growM);
+    else dets_cml<F, L, false>(tm, A, l, Dre, Dim, dM, growK, growM);
     {
       // static order not safe for this matrix (or forced by the caller): repeat with the pivoted eliminations
       const bool risky = act && ((growK >= P.grow_k_max) || (check && growM >= P.grow_m_max));
@@ -878,8 +879,8 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         double s0 = 0.0, s1 = 0.0;
 #pragma unroll
         for (int i = 0; i < L; i++) {
-          s0 += lds(gsa + 8 * (X::O_RED + (2 * i) * G));
-          s1 += lds(gsa + 8 * (X::O_RED + (2 * i + 1) * G));
+          s0 += lds(A.g + 8 * (X::O_RED + 2 * i) * G);
+          s1 += lds(A.g + 8 * (X::O_RED + 2 * i + 1) * G);
         }
         // only the phase of the determinant is used: bring it to unit scale (a power of two, exact)
         const int ex = (int)((max(abs_hi(Dre), abs_hi(Dim)) >> 20) & 0x7ffu);
@@ -915,10 +916,10 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         Sa = fma(0.5 * adt * mu_s[s], Pm[s] * Pm[s], Sa);
         Q[s] = fma(adt * mu_s[s], Pm[s], Q[s]);
       }
-      __syncwarp();  // region A changes hands: every lane is done with the pivot columns / the previous Hessian
-      pes_cml<F, L, KIND>(cs, gsa, l, act, Q, gq, Va);
+      __syncwarp();  // every lane is done with the previous Hessian
+      pes_cml<F, L, KIND>(cs, A, l, Q, gq, Va);
       __syncwarp();
-      pass_cml<F, L, KIND>(tm, gsa, hma, P, post, adt, pre);
+      pass_cml<F, L, KIND>(tm, A, P, post, adt, pre);
       Sa = fma(-pre, Va, Sa);
 #pragma unroll
       for (int s = 0; s < C; s++) Pm[s] = fma(-pre, gq[s], Pm[s]);
@@ -949,7 +950,7 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
 #pragma unroll
     for (int s = 0; s < NS; s++) {
       double col[N];
-      tmem_ld_f64<N>(tm + s * N * 2, col);
+      tmem_ld_col<F, L>(tm, s, col);
       const int a = l + (s % C) * L, h = s / C;
       if (!valid || (!X::EXACT && a >= F)) continue;
       const double ca = h == 0 ? P.isg[a] : P.sg[a];
@@ -984,8 +985,12 @@ __global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__rest
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool act = lane < X::ACT;
   const int l = act ? lane / G : 0, g = act ? lane - l * G : 0;
-  double *gs = smem + X::NCOEFP + warp * X::WS + g;
-  const uint32_t gsa = (uint32_t)__cvta_generic_to_shared(gs);
+  double *ws = smem + X::NCOEFP + warp * X::WS;
+  LaneAddr A;
+  A.g = (uint32_t)__cvta_generic_to_shared(ws + g);
+  A.hm = 0;
+  A.g0 = g;
+  auto HSv = [&](int e) { return ws[(X::O_HS + e) * G + g]; };
   const long long jj = ((long long)blockIdx.x * kWarpsC + warp) * G + g;
   const bool valid = act && jj < n;
   const long long jl = jj < n ? jj : n - 1;
@@ -995,7 +1000,7 @@ __global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__rest
     const int a = l + s * L;
     Q[s] = (X::EXACT || a < F) ? q[(long long)a * n + jl] * sgv[a] : 0.0;
   }
-  pes_cml<F, L, KIND>(cs, gsa, l, act, Q, gq, Va);
+  pes_cml<F, L, KIND>(cs, A, l, Q, gq, Va);
   __syncwarp();
   double Vt = 0.0;
 #pragma unroll
@@ -1008,12 +1013,12 @@ __global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__rest
     if (!X::EXACT && a >= F) continue;
     gout[(long long)a * n + jl] = gq[s] * sgv[a];
     if (KIND != SC_IVR_PES_QFF) {
-      for (int b = 0; b < F; b++) H[((long long)a * F + b) * n + jl] = (b == a) ? gs[X::O_HS + a * G] * sgv[a] * sgv[a] : 0.0;
+      for (int b = 0; b < F; b++) H[((long long)a * F + b) * n + jl] = (b == a) ? HSv(a) * sgv[a] * sgv[a] : 0.0;
     } else {
 #pragma unroll
       for (int d = 0; d < X::ND; d++) {
         const int b = (a + d) % F;
-        const double h = gs[X::O_HS + (d * F + a) * G] * sgv[a] * sgv[b];
+        const double h = HSv(d * F + a) * sgv[a] * sgv[b];
         H[((long long)a * F + b) * n + jl] = h;
         H[((long long)b * F + a) * n + jl] = h;
       }
