@@ -71,6 +71,29 @@ __device__ __forceinline__ void sts2(uint32_t a, double x, double y) {
 // (ncu: l1tex__data_pipe_lsu_wavefronts_mem_shared, profiles/r02b)
 __device__ __forceinline__ double bcast(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
+// Keeps warps in the same code region so that they share the instruction-cache lines they fetch (the time step is ~60 KB
+// of straight-line code; ncu: every 128-byte line costs the fetching warp a "no instruction" bubble).
+//   SCI_CML_SYNC = 1: CTA barrier once per time step; 2: barrier of the two warps of a scheduler once per step;
+//   3: the same at every phase boundary
+#ifndef SCI_CML_SYNC
+#define SCI_CML_SYNC 1
+#endif
+__device__ __forceinline__ void pair_sync() {
+  const int id = 1 + ((threadIdx.x >> 5) & 3);
+  asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory");
+}
+__device__ __forceinline__ void step_sync() {
+  if (SCI_CML_SYNC == 1) __syncthreads();
+  if (SCI_CML_SYNC == 2 || SCI_CML_SYNC == 3) pair_sync();
+  if (SCI_CML_SYNC >= 4) {  // the warps 0-3 and 4-7 as two groups (one warp of each per scheduler)
+    const int id = 5 + (threadIdx.x >> 7);
+    asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory");
+  }
+}
+__device__ __forceinline__ void phase_sync() {
+  if (SCI_CML_SYNC == 3) pair_sync();
+}
+
 template <int F, int L>
 struct Cml {
   static constexpr int C = (F + L - 1) / L;   // modes per lane
@@ -302,14 +325,17 @@ template <int F, int L, int KIND>
 __device__ __forceinline__ void pass_cml(uint32_t tm, const LaneAddr &A, const PropParams &P, double post, double adt, double pre) {
   using X = Cml<F, L>;
   constexpr int C = X::C;
-#pragma unroll
+  // a real loop: the second half runs from the instruction-cache lines the first one fetched
+#pragma unroll 1
   for (int h = 0; h < 2; h++) {
+    const uint32_t tmh = tm + h * C * F * 2;
+    const uint32_t hmh = A.hm + h * (X::HMH * 256);
     double sp[C * F], sq[C * F];
-    tmem_ld_f64<C * F>(tm + h * C * F * 2, sp);
-    tmem_ld_f64<C * F>(tm + (X::TH + h * C * F) * 2, sq);
+    tmem_ld_f64<C * F>(tmh, sp);
+    tmem_ld_f64<C * F>(tmh + X::TH * 2, sq);
     double hp[X::HMH];
 #pragma unroll
-    for (int e = 0; e < C * F; e += 2) lds2(A.hm + X::hm(h * X::HMH + e), hp[e], hp[e + 1]);
+    for (int e = 0; e < C * F; e += 2) lds2(hmh + X::hm(e), hp[e], hp[e + 1]);
     double dP[C][F], dQ[C][F], HM[C][F];
 #pragma unroll
     for (int c = 0; c < C; c++)
@@ -328,9 +354,9 @@ __device__ __forceinline__ void pass_cml(uint32_t tm, const LaneAddr &A, const P
       }
 #pragma unroll
     for (int e = 0; e < C * F; e += 2)
-      sts2(A.hm + X::hm(h * X::HMH + e), HM[e / F][e % F], (e + 1 < C * F) ? HM[(e + 1) / F][(e + 1) % F] : 0.0);
-    tmem_st_f64<C * F>(tm + h * C * F * 2, sp);
-    tmem_st_f64<C * F>(tm + (X::TH + h * C * F) * 2, sq);
+      sts2(hmh + X::hm(e), HM[e / F][e % F], (e + 1 < C * F) ? HM[(e + 1) / F][(e + 1) % F] : 0.0);
+    tmem_st_f64<C * F>(tmh, sp);
+    tmem_st_f64<C * F>(tmh + X::TH * 2, sq);
   }
 }
 
@@ -437,6 +463,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
     }
   }
   // ---- phase B: rows F..2F-1 (W[s][i] is row F + i) ----
+  phase_sync();
   double W[NS][F];
   {
     double st[NS * F];
@@ -488,6 +515,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
       Ki[s][i] = c2p[i] - c1q[i];  // dP2 - dQ1
     }
   }
+  phase_sync();
   double Rr = 1.0, Ri = 0.0;
   unsigned gk = 0u;
   double pc[F], r = 1.0;
@@ -832,6 +860,7 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
   const int nsteps = P.nsteps;
 #pragma unroll 1
   for (int c = 0;; c++) {
+    step_sync();
     const bool last = (c == nsteps);
     const bool check = (det_count == 0) || last;  // warp-uniform
     // a6 (Eq. 3): the lane's share of ln<chi|pq> and of the phase S + arg<chi|pq>, at the integer time c
@@ -892,6 +921,10 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre, Dim);
       }
     }
+    if (SCI_CML_SYNC == 5 && c == 0) {  // the second group starts half a time step late: complementary phases per scheduler
+      if (warp >= 4) asm volatile("bar.sync 7, 256;" ::: "memory");
+      else asm volatile("bar.arrive 7, 256;" ::: "memory");
+    }
     // a7: |det M - 1| <= tol and finite, every det_stride steps and at the end
     if (check) {
       // finite <=> exponent field below 0x7ff: one integer maximum over the high words
@@ -907,6 +940,7 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     // a2-a4 (R10, R11): evaluation points of the "kick b_s, drift a_s" composition
 #pragma unroll 1
     for (int e = 0; e < P.npoints; e++) {
+      phase_sync();
       const double post = P.pt_post[e], adt = P.pt_drift[e];
       const double pre = P.pt_pre[(e + 1 == P.npoints) ? 0 : e + 1];
       Sa = fma(-post, Va, Sa);
