@@ -15,7 +15,16 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsc_ivr.so")
 SOURCES = ["api.cu", "propagate.cu", "propagate_cml.cu", "propagate_tpt.cu", "spectrum.cu", "chirp.cu"]
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "tmem_ldst.cuh"), os.path.join(HERE, "..", "include", "sc_ivr.h")]
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "tmem_ldst.cuh"), os.path.join(CSRC, "cml_table.h"),
+           os.path.join(HERE, "..", "include", "sc_ivr.h")]
+
+
+def cml_table():
+    """(F, L) rows of csrc/cml_table.h: propagate_cml.cu is compiled once per row (-DSCI_CML_INST_F, -DSCI_CML_INST_L)."""
+    import re
+    with open(os.path.join(CSRC, "cml_table.h")) as f:
+        line = [ln for ln in f if ln.startswith("#define SCI_CML_FOR_EACH")][0]
+    return [(int(a), int(b)) for a, b in re.findall(r"X\((\d+),\s*(\d+)\)", line)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 
@@ -39,11 +48,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(objdir, exist_ok=True)
     nvcc = _nvcc()
     jobs = []
-    for src in SOURCES:
+    units = [(src, src.replace(".cu", ".o"), []) for src in SOURCES]
+    units += [("propagate_cml.cu", f"propagate_cml_f{f}.o", [f"-DSCI_CML_INST_F={f}", f"-DSCI_CML_INST_L={l}"]) for f, l in cml_table()]
+    for src, obj, flags in units:
         s = os.path.join(CSRC, src)
-        o = os.path.join(objdir, src.replace(".cu", ".o"))
+        o = os.path.join(objdir, obj)
         if force or _stale(o, [s] + HEADERS):
-            jobs.append([nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
+            jobs.append([nvcc] + NVCC_FLAGS + flags + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
 
     def run(cmd):
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -52,11 +63,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return r.stderr
 
     if jobs:
-        with ThreadPoolExecutor(max_workers=len(jobs)) as ex:
+        with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
             for out in ex.map(run, jobs):
                 if verbose:
                     sys.stderr.write(out)
-    objs = [os.path.join(objdir, s.replace(".cu", ".o")) for s in SOURCES]
+    objs = [os.path.join(objdir, obj) for _, obj, _ in units]
     if force or jobs or _stale(LIB, objs):
         run([nvcc, "-shared", "-o", LIB] + objs)
     return LIB

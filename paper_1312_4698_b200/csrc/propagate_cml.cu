@@ -25,13 +25,18 @@
 #include "common.cuh"
 #include "tmem_ldst.cuh"
 
-namespace {
+#include "cml_table.h"
 
 #ifndef SCI_CML_WARPS
 #define SCI_CML_WARPS 8
 #endif
 constexpr int kWarpsC = SCI_CML_WARPS;
 constexpr int kThreadsC = kWarpsC * 32;
+
+#ifdef SCI_CML_INST_F
+// ======== one (F, L) instantiation per translation unit (build.py compiles this file once per row of cml_table.h) ========
+namespace {
+
 
 __device__ __forceinline__ double rcp_nr2(double x) {
   // MUFU.RCP64H seed (2^-23 relative) + two Newton steps: ~1 ulp for normal x, no slow path.  One step (2^-46) is not
@@ -146,6 +151,23 @@ struct Cml {
     return s >= C || ((s * L + L - 1 < F - 1 ? s * L + L - 1 : F - 1) > k);
   }
 };
+
+// store in chunks of at most WMAX 32-bit columns: a tcgen05.st needs its source in consecutive registers, and gathering
+// 54 of them costs a register move each; short chunks take the values where they are
+#ifndef SCI_CML_ST_W
+#define SCI_CML_ST_W 128
+#endif
+template <int ND, int WMAX>
+__device__ __forceinline__ void tmem_st_f64_w(uint32_t taddr, const double (&d)[ND]) {
+  uint32_t v[2 * ND];
+#pragma unroll
+  for (int i = 0; i < ND; i++) {
+    v[2 * i] = (uint32_t)__double2loint(d[i]);
+    v[2 * i + 1] = (uint32_t)__double2hiint(d[i]);
+  }
+  tmem_st_issue<2 * ND, 0, WMAX>(taddr, v);
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
 
 // one column of M from / to the lane's tensor memory: rows 0..F-1 (dP) and F..2F-1 (dQ) live in different halves
 template <int F, int L>
@@ -355,8 +377,8 @@ __device__ __forceinline__ void pass_cml(uint32_t tm, const LaneAddr &A, const P
 #pragma unroll
     for (int e = 0; e < C * F; e += 2)
       sts2(hmh + X::hm(e), HM[e / F][e % F], (e + 1 < C * F) ? HM[(e + 1) / F][(e + 1) % F] : 0.0);
-    tmem_st_f64<C * F>(tmh, sp);
-    tmem_st_f64<C * F>(tmh + X::TH * 2, sq);
+    tmem_st_f64_w<C * F, SCI_CML_ST_W>(tmh, sp);
+    tmem_st_f64_w<C * F, SCI_CML_ST_W>(tmh + X::TH * 2, sq);
   }
 }
 
@@ -1150,8 +1172,33 @@ size_t pack_cml(int kind, const double *c, const double *gamma, double *out) {
 
 }  // namespace
 
-// (F, L) pairs served by this kernel; every other F >= 4 stays on the one-mode-per-lane kernel of propagate.cu
-#define SCI_CML_FOR_EACH(X) X(9, 3)
+#define SCI_CAT2(a, b) a##b
+#define SCI_CAT(a, b) SCI_CAT2(a, b)
+
+size_t SCI_CAT(sci_cml_pack_f, SCI_CML_INST_F)(int kind, const double *c, const double *gamma, double *out) {
+  return pack_cml<SCI_CML_INST_F, SCI_CML_INST_L>(kind, c, gamma, out);
+}
+
+cudaError_t SCI_CAT(sci_cml_prop_f, SCI_CML_INST_F)(int kind, const PropParams &P, cudaStream_t st) {
+  return kind == SC_IVR_PES_QFF ? launch_prop_cml<SCI_CML_INST_F, SCI_CML_INST_L, SC_IVR_PES_QFF>(P, st)
+                                : launch_prop_cml<SCI_CML_INST_F, SCI_CML_INST_L, SC_IVR_PES_MORSE_UNCOUPLED>(P, st);
+}
+
+cudaError_t SCI_CAT(sci_cml_pes_f, SCI_CML_INST_F)(int kind, const double *coef, const double *sg, const double *q, long long n,
+                                                   double *V, double *g, double *H, cudaStream_t st) {
+  return kind == SC_IVR_PES_QFF ? launch_pes_cml<SCI_CML_INST_F, SCI_CML_INST_L, SC_IVR_PES_QFF>(coef, sg, q, n, V, g, H, st)
+                                : launch_pes_cml<SCI_CML_INST_F, SCI_CML_INST_L, SC_IVR_PES_MORSE_UNCOUPLED>(coef, sg, q, n, V, g, H, st);
+}
+
+#else
+// ======== dispatcher ========================================================================================================
+#define X(f, l)                                                                                                      \
+  size_t sci_cml_pack_f##f(int kind, const double *c, const double *gamma, double *out);                             \
+  cudaError_t sci_cml_prop_f##f(int kind, const PropParams &P, cudaStream_t st);                                     \
+  cudaError_t sci_cml_pes_f##f(int kind, const double *coef, const double *sg, const double *q, long long n, double *V, \
+                               double *g, double *H, cudaStream_t st);
+SCI_CML_FOR_EACH(X)
+#undef X
 
 int sci_cml_lanes(int F) {
   switch (F) {
@@ -1169,7 +1216,7 @@ int sci_cml_traj_per_block(int F) {
 
 size_t sci_cml_pack_coeffs(int F, int kind, const double *c, const double *gamma, double *out) {
   switch (F) {
-#define X(f, l) case f: return pack_cml<f, l>(kind, c, gamma, out);
+#define X(f, l) case f: return sci_cml_pack_f##f(kind, c, gamma, out);
     SCI_CML_FOR_EACH(X)
 #undef X
   }
@@ -1177,9 +1224,8 @@ size_t sci_cml_pack_coeffs(int F, int kind, const double *c, const double *gamma
 }
 
 cudaError_t sci_cml_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st) {
-  const bool qff = kind == SC_IVR_PES_QFF;
   switch (F) {
-#define X(f, l) case f: return qff ? launch_prop_cml<f, l, SC_IVR_PES_QFF>(P, st) : launch_prop_cml<f, l, SC_IVR_PES_MORSE_UNCOUPLED>(P, st);
+#define X(f, l) case f: return sci_cml_prop_f##f(kind, P, st);
     SCI_CML_FOR_EACH(X)
 #undef X
   }
@@ -1188,12 +1234,11 @@ cudaError_t sci_cml_launch_propagate(int F, int kind, const PropParams &P, cudaS
 
 cudaError_t sci_cml_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q, long long n,
                                     double *V, double *g, double *H, cudaStream_t st) {
-  const bool qff = kind == SC_IVR_PES_QFF;
   switch (F) {
-#define X(f, l) case f: return qff ? launch_pes_cml<f, l, SC_IVR_PES_QFF>(coef, sg, q, n, V, g, H, st) \
-                                   : launch_pes_cml<f, l, SC_IVR_PES_MORSE_UNCOUPLED>(coef, sg, q, n, V, g, H, st);
+#define X(f, l) case f: return sci_cml_pes_f##f(kind, coef, sg, q, n, V, g, H, st);
     SCI_CML_FOR_EACH(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
+#endif
