@@ -76,28 +76,13 @@ __device__ __forceinline__ void sts2(uint32_t a, double x, double y) {
 // (ncu: l1tex__data_pipe_lsu_wavefronts_mem_shared, profiles/r02b)
 __device__ __forceinline__ double bcast(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
-// Keeps warps in the same code region so that they share the instruction-cache lines they fetch (the time step is ~60 KB
-// of straight-line code; ncu: every 128-byte line costs the fetching warp a "no instruction" bubble).
-//   SCI_CML_SYNC = 1: CTA barrier once per time step; 2: barrier of the two warps of a scheduler once per step;
-//   3: the same at every phase boundary
+// Optional barriers that keep the warps of a CTA in step (SCI_CML_SYNC = 1: one CTA barrier per time step; 6: the warps 4..
+// run half a time step behind the warps 0..3; 7: both).  Measured on config 4 (profiles/r02): none of them pays once the
+// launch is balanced (219 cycles per trajectory-step per SM without, 232 / 222 / 240 with), so the default is 0.
 #ifndef SCI_CML_SYNC
-#define SCI_CML_SYNC 1
+#define SCI_CML_SYNC 0
 #endif
-__device__ __forceinline__ void pair_sync() {
-  const int id = 1 + ((threadIdx.x >> 5) & 3);
-  asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory");
-}
-__device__ __forceinline__ void step_sync() {
-  if (SCI_CML_SYNC == 1) __syncthreads();
-  if (SCI_CML_SYNC == 2 || SCI_CML_SYNC == 3) pair_sync();
-  if (SCI_CML_SYNC >= 4) {  // the warps 0-3 and 4-7 as two groups (one warp of each per scheduler)
-    const int id = 5 + (threadIdx.x >> 7);
-    asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory");
-  }
-}
-__device__ __forceinline__ void phase_sync() {
-  if (SCI_CML_SYNC == 3) pair_sync();
-}
+__device__ __forceinline__ void cta_sync(int nthreads) { asm volatile("bar.sync 0, %0;" ::"r"(nthreads) : "memory"); }
 
 template <int F, int L>
 struct Cml {
@@ -485,7 +470,6 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
     }
   }
   // ---- phase B: rows F..2F-1 (W[s][i] is row F + i) ----
-  phase_sync();
   double W[NS][F];
   {
     double st[NS * F];
@@ -537,7 +521,6 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
       Ki[s][i] = c2p[i] - c1q[i];  // dP2 - dQ1
     }
   }
-  phase_sync();
   double Rr = 1.0, Ri = 0.0;
   unsigned gk = 0u;
   double pc[F], r = 1.0;
@@ -842,7 +825,14 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
 #pragma unroll
   for (int i = 0; i < L; i++) gmask |= 1u << (i * G + g);
 
-  const long long jj = ((long long)blockIdx.x * kWarpsC + warp) * G + g;
+  // balanced launch: CTA b runs cta_warps (+1 for the first cta_warps_rem CTAs) warps of G trajectories each, so that every SM
+  // gets the same number of warp-rounds (a grid of full CTAs leaves the last wave almost empty: 131072 trajectories are
+  // 11.07 waves of 148 x 80)
+  const int nw = P.cta_warps + ((int)blockIdx.x < P.cta_warps_rem ? 1 : 0);
+  const int nthr = nw * 32;
+  if (warp >= nw) return;  // after the barrier above; the barriers below count nthr threads
+  const long long w0 = (long long)blockIdx.x * P.cta_warps + min((int)blockIdx.x, P.cta_warps_rem);
+  const long long jj = (w0 + warp) * G + g;
   const bool valid = act && jj < P.nb;
   const long long jl = jj < P.nb ? jj : P.nb - 1;  // tail groups recompute the last trajectory and store nothing
   const long long jg = P.j0 + jl;
@@ -882,7 +872,12 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
   const int nsteps = P.nsteps;
 #pragma unroll 1
   for (int c = 0;; c++) {
-    step_sync();
+    if (SCI_CML_SYNC >= 6) {
+      if (c == 0 && warp >= 4) asm volatile("bar.sync 7, %0;" ::"r"(nthr) : "memory");
+      if (SCI_CML_SYNC == 7 && warp < 4 && c > 0) cta_sync(nthr);
+    } else if (SCI_CML_SYNC == 1) {
+      cta_sync(nthr);
+    }
     const bool last = (c == nsteps);
     const bool check = (det_count == 0) || last;  // warp-uniform
     // a6 (Eq. 3): the lane's share of ln<chi|pq> and of the phase S + arg<chi|pq>, at the integer time c
@@ -943,9 +938,11 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
         if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre, Dim);
       }
     }
-    if (SCI_CML_SYNC == 5 && c == 0) {  // the second group starts half a time step late: complementary phases per scheduler
-      if (warp >= 4) asm volatile("bar.sync 7, 256;" ::: "memory");
-      else asm volatile("bar.arrive 7, 256;" ::: "memory");
+    if (SCI_CML_SYNC >= 6) {
+      // the warps 4.. run half a time step behind the warps 0..3 (one of each per scheduler): while one does the
+      // eliminations the other does the PES and the pass
+      if (c == 0 && warp < 4) asm volatile("bar.arrive 7, %0;" ::"r"(nthr) : "memory");
+      if (SCI_CML_SYNC == 7 && warp >= 4 && !last) cta_sync(nthr);
     }
     // a7: |det M - 1| <= tol and finite, every det_stride steps and at the end
     if (check) {
@@ -962,7 +959,6 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     // a2-a4 (R10, R11): evaluation points of the "kick b_s, drift a_s" composition
 #pragma unroll 1
     for (int e = 0; e < P.npoints; e++) {
-      phase_sync();
       const double post = P.pt_post[e], adt = P.pt_drift[e];
       const double pre = P.pt_pre[(e + 1 == P.npoints) ? 0 : e + 1];
       Sa = fma(-post, Va, Sa);
@@ -1020,7 +1016,7 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     }
   }
   tmem_fence_before_sync();
-  __syncthreads();
+  cta_sync(nthr);
   if (warp == 0) tmem_free_all(tm_base);
 }
 
@@ -1094,9 +1090,16 @@ cudaError_t launch_prop_cml(const PropParams &P, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) attr_dev_mask[dev] = 1;
   }
-  const int tpb = kWarpsC * X::G;
-  const long long blocks = (P.nb + tpb - 1) / tpb;
-  k_propagate_cml<F, L, KIND><<<(unsigned)blocks, kThreadsC, X::SMEM, st>>>(P);
+  int sm = 0;
+  e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return e;
+  const long long W = (P.nb + X::G - 1) / X::G;                                  // warps of work
+  const long long rounds = (W + (long long)sm * kWarpsC - 1) / ((long long)sm * kWarpsC);
+  const long long blocks = W < rounds * sm ? W : rounds * sm;                   // one CTA per SM and round
+  PropParams Q = P;
+  Q.cta_warps = (int)(W / blocks);
+  Q.cta_warps_rem = (int)(W % blocks);
+  k_propagate_cml<F, L, KIND><<<(unsigned)blocks, kThreadsC, X::SMEM, st>>>(Q);
   return cudaGetLastError();
 }
 
