@@ -44,15 +44,22 @@ __device__ __forceinline__ double rcp_nr2(double x) {
   // 1e-14 move |det M - 1| across the 1e-6 threshold where the oracle's exact multipliers do not (152 of 131072
   // trajectories of config 4 change their flag).
 #ifndef SCI_CML_RCP_NR
-#define SCI_CML_RCP_NR 2
+#define SCI_CML_RCP_NR 3
 #endif
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+#if SCI_CML_RCP_NR == 3
+  // cubic step: r (1 + e + e^2), e = 1 - x r = 2^-23  ->  2^-69 before rounding, three dependent FMAs instead of four
+  const double e = fma(-x, r, 1.0);
+  const double t = fma(e, e, e);
+  r = fma(r, t, r);
+#else
 #pragma unroll
   for (int it = 0; it < SCI_CML_RCP_NR; it++) {
     const double e = fma(-x, r, 1.0);
     r = fma(r, e, r);
   }
+#endif
   return r;
 }
 
@@ -870,6 +877,7 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
   bool good = true;
   int det_count = 0;  // steps until the next check
   const int nsteps = P.nsteps;
+  const bool has_raw = P.raw != nullptr, has_pq = P.pq_steps != nullptr;
 #pragma unroll 1
   for (int c = 0;; c++) {
     if (SCI_CML_SYNC >= 6) {
@@ -881,18 +889,23 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
     const bool last = (c == nsteps);
     const bool check = (det_count == 0) || last;  // warp-uniform
     // a6 (Eq. 3): the lane's share of ln<chi|pq> and of the phase S + arg<chi|pq>, at the integer time c
-    if (P.raw != nullptr) {
+    if (has_raw) {  // uniform branches only: a divergent one costs reconvergence barriers and an instruction-fetch restart
       double oa = 0.0, ob = Sa;
 #pragma unroll
       for (int s = 0; s < C; s++) {
-        if (!X::EXACT && l + s * L >= F) continue;
+        const bool real = X::EXACT || l + s * L < F;
         const double dq = Qeq_s[s] - Q[s], dp = Peq_s[s] - Pm[s];
-        oa = fma(-0.25, fma(dq, dq, dp * dp), oa);
-        ob = fma(0.5 * (Peq_s[s] + Pm[s]), dq, ob);
-        if (P.pq_steps != nullptr && valid)
-          P.pq_steps[((long long)c * F + (l + s * L)) * P.raw_stride + jj] = make_double2(Pm[s], Q[s]);
+        const double ta = fma(-0.25, fma(dq, dq, dp * dp), oa), tb = fma(0.5 * (Peq_s[s] + Pm[s]), dq, ob);
+        oa = real ? ta : oa;
+        ob = real ? tb : ob;
       }
-      if (P.raw_plain) {  // several reference states: the record carries S alone, (P, Q) of the step go out beside it
+      if (has_pq) {  // several reference states: the record carries S alone, (P, Q) of the step go out beside it
+#pragma unroll
+        for (int s = 0; s < C; s++)
+          if (valid && (X::EXACT || l + s * L < F))
+            P.pq_steps[((long long)c * F + (l + s * L)) * P.raw_stride + jj] = make_double2(Pm[s], Q[s]);
+      }
+      if (P.raw_plain) {
         oa = 0.0;
         ob = Sa;
       }
@@ -919,24 +932,18 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
       }
     }
     // a8 input record, written by the lane that holds the last pivots
-    if (P.raw != nullptr) {
+    if (has_raw) {
       __syncwarp();
-      if (l == lw) {
-        double s0 = 0.0, s1 = 0.0;
+      double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-        for (int i = 0; i < L; i++) {
-          s0 += lds(A.g + 8 * (X::O_RED + 2 * i) * G);
-          s1 += lds(A.g + 8 * (X::O_RED + 2 * i + 1) * G);
-        }
-        // only the phase of the determinant is used: bring it to unit scale (a power of two, exact)
-        const int ex = (int)((max(abs_hi(Dre), abs_hi(Dim)) >> 20) & 0x7ffu);
-        if (ex > 0 && ex < 0x7fe) {
-          const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex)
-          Dre *= sc;
-          Dim *= sc;
-        }
-        if (valid) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre, Dim);
+      for (int i = 0; i < L; i++) {
+        s0 += lds(A.g + 8 * (X::O_RED + 2 * i) * G);
+        s1 += lds(A.g + 8 * (X::O_RED + 2 * i + 1) * G);
       }
+      // only the phase of the determinant is used: bring it to unit scale (a power of two, exact)
+      const int ex = (int)((max(abs_hi(Dre), abs_hi(Dim)) >> 20) & 0x7ffu);
+      const double sc = (ex > 0 && ex < 0x7fe) ? __hiloint2double((0x7fe - ex) << 20, 0) : 1.0;  // 2^(1023 - ex)
+      if (valid && l == lw) P.raw[(long long)c * P.raw_stride + jj] = make_double4(s0, s1, Dre * sc, Dim * sc);
     }
     if (SCI_CML_SYNC >= 6) {
       // the warps 4.. run half a time step behind the warps 0..3 (one of each per scheduler): while one does the
