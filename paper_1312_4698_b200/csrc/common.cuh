@@ -44,7 +44,7 @@ struct PropParams {
   // then formed per reference state by the z assembly
   double2 *pq_steps;
   int raw_plain;
-  int cta_warps, cta_warps_rem;  // propagate_cml.cu: set by the launcher (balanced CTAs)
+  int cta_full, cta_warps, cta_warps_rem;  // propagate_cml.cu: launch shape, set by the launcher
   unsigned long long *fb_count;  // may be NULL: number of trajectory-steps repeated with the pivoted eliminations
   unsigned char *good;           // [nb]; may be NULL
   // debug outputs (may be NULL), indexed by the GLOBAL trajectory number j0 + jj with stride `stride`

@@ -832,13 +832,16 @@ __global__ void __launch_bounds__(kThreadsC, 1) k_propagate_cml(const __grid_con
 #pragma unroll
   for (int i = 0; i < L; i++) gmask |= 1u << (i * G + g);
 
-  // balanced launch: CTA b runs cta_warps (+1 for the first cta_warps_rem CTAs) warps of G trajectories each, so that every SM
-  // gets the same number of warp-rounds (a grid of full CTAs leaves the last wave almost empty: 131072 trajectories are
-  // 11.07 waves of 148 x 80)
-  const int nw = P.cta_warps + ((int)blockIdx.x < P.cta_warps_rem ? 1 : 0);
+  // launch shape: cta_full CTAs of kWarpsC warps (whole rounds of one CTA per SM), then the warps that are left spread
+  // evenly over one more CTA per SM (cta_warps, +1 for the first cta_warps_rem of them): a step of a CTA takes as long as
+  // that of its busiest scheduler, so a last round with one warp per scheduler costs 0.7 of a full one and a nearly
+  // empty grid tail a whole one (131072 trajectories of config 4 are 11.07 rounds of 148 x 80)
+  const int bt = (int)blockIdx.x - P.cta_full;
+  const int nw = bt < 0 ? kWarpsC : P.cta_warps + (bt < P.cta_warps_rem ? 1 : 0);
   const int nthr = nw * 32;
   if (warp >= nw) return;  // after the barrier above; the barriers below count nthr threads
-  const long long w0 = (long long)blockIdx.x * P.cta_warps + min((int)blockIdx.x, P.cta_warps_rem);
+  const long long w0 = bt < 0 ? (long long)blockIdx.x * kWarpsC
+                              : (long long)P.cta_full * kWarpsC + (long long)bt * P.cta_warps + min(bt, P.cta_warps_rem);
   const long long jj = (w0 + warp) * G + g;
   const bool valid = act && jj < P.nb;
   const long long jl = jj < P.nb ? jj : P.nb - 1;  // tail groups recompute the last trajectory and store nothing
@@ -1101,12 +1104,15 @@ cudaError_t launch_prop_cml(const PropParams &P, cudaStream_t st) {
   e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
   if (e != cudaSuccess) return e;
   const long long W = (P.nb + X::G - 1) / X::G;                                  // warps of work
-  const long long rounds = (W + (long long)sm * kWarpsC - 1) / ((long long)sm * kWarpsC);
-  const long long blocks = W < rounds * sm ? W : rounds * sm;                   // one CTA per SM and round
+  const long long per_round = (long long)sm * kWarpsC;
+  const long long full = W / per_round * sm;                                     // CTAs of whole rounds
+  const long long left = W - full * kWarpsC;                                     // warps of the last, partial round
+  const long long tail = left < sm ? left : sm;
   PropParams Q = P;
-  Q.cta_warps = (int)(W / blocks);
-  Q.cta_warps_rem = (int)(W % blocks);
-  k_propagate_cml<F, L, KIND><<<(unsigned)blocks, kThreadsC, X::SMEM, st>>>(Q);
+  Q.cta_full = (int)full;
+  Q.cta_warps = tail ? (int)(left / tail) : 0;
+  Q.cta_warps_rem = tail ? (int)(left % tail) : 0;
+  k_propagate_cml<F, L, KIND><<<(unsigned)(full + tail), kThreadsC, X::SMEM, st>>>(Q);
   return cudaGetLastError();
 }
 
