@@ -9,6 +9,8 @@
 #include <new>
 #include <vector>
 
+#include <stdlib.h>
+
 #include "common.cuh"
 
 namespace {
