@@ -172,7 +172,7 @@ bool chirp_applies(const sc_ivr_ctx *ctx, const double *E, int k, double *e0, do
   return uniform_grid(E, k, e0, de);
 }
 
-// kernel A: one thread per trajectory for F <= SCI_TPT_MAXF, F lanes per trajectory above
+// kernel A: one thread per trajectory for F <= SCI_TPT_MAXF, C modes per lane (cml_table.h) above
 cudaError_t launch_kernel_a(const sc_ivr_ctx *ctx, const PropParams &P, cudaStream_t st) {
   if (ctx->F <= SCI_TPT_MAXF) {
     TptParams TP;
@@ -180,8 +180,7 @@ cudaError_t launch_kernel_a(const sc_ivr_ctx *ctx, const PropParams &P, cudaStre
     memcpy(TP.coef, ctx->tpt_coef, sizeof(TP.coef));
     return sci_tpt_launch_propagate(ctx->F, ctx->kind, TP, st);
   }
-  if (sci_cml_lanes(ctx->F)) return sci_cml_launch_propagate(ctx->F, ctx->kind, P, st);
-  return sci_launch_propagate(ctx->F, ctx->kind, P, st);
+  return sci_cml_launch_propagate(ctx->F, ctx->kind, P, st);
 }
 
 struct StageTimer {
@@ -293,12 +292,14 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
       rc = fail(nullptr, SC_IVR_ECUDA, "cannot query the CUDA device");
       break;
     }
-    const bool cml = F > SCI_TPT_MAXF && sci_cml_lanes(F) != 0;
-    const size_t nc = cml ? sci_cml_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr)
-                          : sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr);
+    const bool cml = F > SCI_TPT_MAXF;
+    if (cml && sci_cml_lanes(F) == 0) {
+      rc = fail(nullptr, SC_IVR_EINVAL, "F = %d has no kernel (cml_table.h)", F);
+      break;
+    }
+    const size_t nc = cml ? sci_cml_pack_coeffs(F, (int)kind, pes_coeffs, gamma, nullptr) : 0;
     std::vector<double> packed(nc + F);  // sqrt(gamma) rides behind the coefficients (for sc_ivr_eval_pes)
     if (cml) sci_cml_pack_coeffs(F, (int)kind, pes_coeffs, gamma, packed.data());
-    else sci_pack_coeffs(F, (int)kind, pes_coeffs, gamma, packed.data());
     for (int a = 0; a < F; a++) packed[nc + a] = sqrt(gamma[a]);
     ctx->n_coef = nc;
     if ((ce = cudaMalloc(&ctx->d_coef, sizeof(double) * (nc + F))) != cudaSuccess ||
@@ -310,10 +311,8 @@ sc_ivr_status sc_ivr_create(sc_ivr_ctx **out, int F, sc_ivr_pes_kind kind, const
       memset(ctx->tpt_coef, 0, sizeof(ctx->tpt_coef));
       sci_tpt_pack_coeffs(F, (int)kind, pes_coeffs, gamma, ctx->tpt_coef);
       ctx->wave = (long long)ctx->sm_count * sci_tpt_blocks_per_sm(F, (int)kind) * sci_tpt_traj_per_block();
-    } else if (cml) {
-      ctx->wave = (long long)ctx->sm_count * sci_cml_traj_per_block(F);  // one CTA per SM
     } else {
-      ctx->wave = (long long)ctx->sm_count * sci_prop_blocks_per_sm(F, (int)kind) * sci_prop_traj_per_block(F);
+      ctx->wave = (long long)ctx->sm_count * sci_cml_traj_per_block(F);  // one CTA per SM
     }
   } while (0);
   if (rc != SC_IVR_OK) {
@@ -563,12 +562,8 @@ sc_ivr_status sc_ivr_eval_pes(sc_ivr_ctx *ctx, const double *q, long long n, dou
     CU(sci_tpt_launch_eval_pes(ctx->F, ctx->kind, TP, q, n, V_out, g_out, H_out, (cudaStream_t)cuda_stream));
     return SC_IVR_OK;
   }
-  if (sci_cml_lanes(ctx->F))
-    CU(sci_cml_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
-                               (cudaStream_t)cuda_stream));
-  else
-    CU(sci_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
-                           (cudaStream_t)cuda_stream));
+  CU(sci_cml_launch_eval_pes(ctx->F, ctx->kind, ctx->d_coef, ctx->d_coef + ctx->n_coef, q, n, V_out, g_out, H_out,
+                             (cudaStream_t)cuda_stream));
   return SC_IVR_OK;
 }
 

@@ -81,14 +81,6 @@ struct sc_ivr_ctx {
   size_t ev_used;
 };
 
-// kernel A launchers (propagate.cu)
-int sci_prop_traj_per_block(int F);
-int sci_prop_blocks_per_sm(int F, int kind);
-size_t sci_pack_coeffs(int F, int kind, const double *coeffs, const double *gamma, double *out /*may be NULL: size query*/);
-cudaError_t sci_launch_propagate(int F, int kind, const PropParams &P, cudaStream_t st);
-cudaError_t sci_launch_eval_pes(int F, int kind, const double *coef, const double *sg, const double *q,
-                                long long n, double *V, double *g, double *H, cudaStream_t st);
-
 // C-modes-per-lane kernels with the monodromy state in tensor memory (propagate_cml.cu)
 int sci_cml_lanes(int F);  // lanes per trajectory, 0 = F is not served by these kernels
 int sci_cml_traj_per_block(int F);

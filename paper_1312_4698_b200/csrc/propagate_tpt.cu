@@ -307,7 +307,8 @@ __global__ void __launch_bounds__(kTptThreads) k_propagate_tpt(const __grid_cons
         }
       unsigned growM;
       double dM = det_static_real<2 * F>(A, growM);
-      if (growM >= P.grow_m_max) {
+      // a rejection by the fixed-order elimination is confirmed by the pivoted one before it sticks (see propagate_cml.cu)
+      if (growM >= P.grow_m_max || (good && !(fabs(dM - 1.0) <= P.det_tol))) {
         double buf[4 * F * F];
 #pragma unroll
         for (int i = 0; i < F; i++)
