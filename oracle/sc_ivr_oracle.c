@@ -459,7 +459,7 @@ int sc_ivr_oracle_propagate(int F, int kind, const double *coeffs, long ncoef, c
  * fourier_mode 0 ("exact"): the definition, one cexp per term.
  * fourier_mode 1 ("recur"): the same sum with the twiddle advanced by w <- w r, r = e^{i E_i dt},
  *   re-seeded with an exact cexp every 256 steps (error <= 256 eps per term); pinned to mode 0 by
- *   tests/test_oracle_fourier.py.  Used where mode 0 would take hours.
+ *   tests/test_oracle_pins.py (test_p10_*).  Used where mode 0 would take hours.
  * Asq[i] += wj * |A_j(E_i)|^2 for one trajectory.
  */
 static void fourier_accumulate(const double *z, int nsteps, double dt, const double *E, int k, int mode,

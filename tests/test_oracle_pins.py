@@ -463,11 +463,28 @@ def test_p12_morse_levels_loose(oracle):
     assert abs(Ecm[np.argmax(I)] - lev[0]) <= 3 * bin_w
 
 
+def _line_check(spec_single, spec_combo, factors, om, T, dE, nlines):
+    """Lines of a harmonic spectrum under a rectangular window of length T ("leakage bound"): a line m
+    of power P_m puts at most sqrt(P_m) / ((N + 1) |sin((E_n - E_m) dt / 2)|) <= sqrt(P_m) 2 / (|n - m| om T) of
+    amplitude (Dirichlet kernel) under the line n.  With combination factors f_m on the single-state powers P1_m,
+    the amplitude under line n is sqrt(f_n P1_n) up to the sum of those side lobes; no tuned constants."""
+    idx = [int(round((n + 0.5) * om / dE)) for n in range(nlines)]
+    P1 = np.array([spec_single[i] for i in idx])
+    for n in range(nlines):
+        leak = sum(np.sqrt(factors[m] * P1[m]) * 2.0 / (abs(n - m) * om * T) for m in range(nlines) if m != n)
+        leak += np.sqrt(P1[n]) * sum(2.0 / (abs(n - m) * om * T) for m in range(nlines) if m != n)  # P1_n itself carries side lobes
+        leak *= 1.05                                                                                # lines above the grid (Poisson tail)
+        got, want = np.sqrt(spec_combo[idx[n]]), np.sqrt(factors[n] * P1[n])
+        assert abs(got - want) <= leak, (n, got, want, leak)
+        if factors[n] == 0.0 and P1[n] > 1e-3 * P1.max():
+            assert spec_combo[idx[n]] < 0.02 * P1[n]  # the bound is not vacuous: the line is gone
+
+
 def test_combo_reference_state_parity_selection_rule(oracle):
     """Row f4 (Fig. 4): reference state = combination of coherent states.  Closed-form pin: for a
     1-D harmonic oscillator with gamma = omega, |alpha> + |-alpha> contains only even and |alpha> - |-alpha> only odd
     number states (the mirror image about q_eq), so each combination keeps every second peak of the single-state
-    spectrum, at (n + 1/2) omega~, and removes the others."""
+    spectrum, at (n + 1/2) omega~, with four times its power, and removes the others."""
     om = 0.01
     nsteps, dt = 6000, 2.0  # omega dt = 0.02: the Verlet map is harmonic with omega~ = omega (1 + 1.7e-5)
     E = np.linspace(0.0, 6.0 * om, 601)
@@ -482,17 +499,34 @@ def test_combo_reference_state_parity_selection_rule(oracle):
         assert (ng, rc) == (24, 0)
     I1, rc1 = oracle.run(1, w.pes_kind, w.pes_coeffs, w.gamma, dt, nsteps, w.p0q0, w.chi, E, fourier_mode=0)[::2]
     assert np.allclose(spec["single"], I1, rtol=1e-12, atol=0)  # eps = (1, 0) is the plain reference state
-    mx = spec["single"].max()
-    for n in range(5):
-        i = int(round((n + 0.5) * om / (E[1] - E[0])))
-        keep, kill = ("even", "odd") if n % 2 == 0 else ("odd", "even")
-        if spec["single"][i] > 1e-3 * mx:
-            # what is left is the side-lobe leakage of the two kept neighbours (rectangular window of length T)
-            assert spec[kill][i] < max(2e-3 * spec["single"][i], 1e-3 * mx), (n, spec[kill][i] / spec["single"][i])
-            assert spec[kill][i] < 0.05 * spec["single"][i]
-            # amplitude doubles, power x4 (to the side-lobe leakage of the removed neighbours at finite T)
-            if spec["single"][i] > 2e-2 * mx:
-                assert abs(spec[keep][i] / spec["single"][i] / 4.0 - 1.0) < 3e-2
+    # <n|-alpha> = (-1)^n <n|alpha>: |1 + eps (-1)^n|^2
+    _line_check(spec["single"], spec["even"], [4.0, 0.0, 4.0, 0.0, 4.0, 0.0], om, nsteps * dt, E[1] - E[0], 6)
+    _line_check(spec["single"], spec["odd"], [0.0, 4.0, 0.0, 4.0, 0.0, 4.0], om, nsteps * dt, E[1] - E[0], 6)
+
+
+def test_combo_reference_state_conjugation(oracle):
+    """The conjugate in <chi| = sum_m conj(eps_m) <p_m q_m| (reference_overlap in the oracle), pinned by a
+    closed form that a slip eps <-> conj(eps) breaks.  1-D harmonic oscillator, gamma = omega, q_eq = 0; coherent states
+    m = 0: (p_e, 0), i.e. alpha = i p_e / sqrt(2 gamma), and m = 1: (0, -p_e / gamma), i.e. alpha' = i alpha (both have
+    p (q - q_eq) = 0, so Eq. 3's state is the Glauber state without an extra phase).  Number-state amplitudes:
+    <n|alpha'> = i^n <n|alpha>, so |chi> = |alpha> + eps |alpha'> carries |1 + eps i^n|^2 times the single-state power of
+    line n: for eps = +i that is (2, 0, 2, 4, 2, 0), for eps = -i it is (2, 4, 2, 0, 2, 4).  With the conjugate dropped the
+    two lists swap: line 1 would survive with four times its power where it must vanish."""
+    om = 0.01
+    nsteps, dt = 6000, 2.0
+    E = np.linspace(0.0, 6.0 * om, 601)
+    w = inputs.make_harmonic([om], ntraj=24, nsteps=nsteps, dt=dt, E=E, seed=3)
+    p_e, q_e, g = w.chi[0], w.chi[1], w.gamma[0]
+    assert abs(q_e) < 1e-15 and abs(g - om) < 1e-15
+    chis = np.array([[p_e, 0.0], [0.0, -p_e / g]])
+    spec = {}
+    for name, eps in (("single", np.array([1.0, 0.0], dtype=complex)), ("plus_i", np.array([1.0, 1.0j])), ("minus_i", np.array([1.0, -1.0j]))):
+        spec[name], ng, rc = oracle.run_combo(1, w.pes_kind, w.pes_coeffs, w.gamma, dt, nsteps, w.p0q0, chis, eps, E, fourier_mode=0)
+        assert (ng, rc) == (24, 0)
+    fac = {"plus_i": [abs(1 + 1j * 1j ** n) ** 2 for n in range(6)], "minus_i": [abs(1 - 1j * 1j ** n) ** 2 for n in range(6)]}
+    assert np.allclose(fac["plus_i"], [2, 0, 2, 4, 2, 0]) and np.allclose(fac["minus_i"], [2, 4, 2, 0, 2, 4])
+    for name in ("plus_i", "minus_i"):
+        _line_check(spec["single"], spec[name], [round(f) * 1.0 for f in fac[name]], om, nsteps * dt, E[1] - E[0], 6)
 
 
 def test_combo_reference_state_brute_force(oracle):
