@@ -116,6 +116,11 @@ long long sc_ivr_min_batch(const sc_ivr_ctx *ctx);
  * reproducible for fixed (inputs, workspace size).  Asynchronous on cuda_stream when n_good_out is
  * NULL (then a batch with no good trajectory yields I_out = 0 and SC_IVR_OK); otherwise the stream
  * is synchronised once at the end and SC_IVR_ENOGOOD is returned when n_good == 0.
+ * Lifetime in the asynchronous case: E is copied to the device with cudaMemcpyAsync on cuda_stream; if it is PINNED host
+ * memory the caller keeps it alive and unmodified until the stream has passed this call (pageable memory is staged before
+ * the call returns).  chi is consumed before the call returns.
+ * Device: the call must be issued with the context's device current (the one that was current in sc_ivr_create);
+ * otherwise SC_IVR_EINVAL.  The same holds for every other entry point that takes a stream.
  */
 sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj,
                          const double *chi, const double *E, int k, double *I_out, long long *n_good_out,
@@ -144,8 +149,9 @@ sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double 
  *   I_out DEVICE [nchi][k]                             E    HOST [k], equally spaced (chirp-z path only)
  *   workspace DEVICE, sc_ivr_multi_workspace_bytes(ctx, ntraj, k, ncs, max_batch); a smaller one (>= one batch of
  *   sc_ivr_min_batch) makes more, smaller batches.  1 <= ncs <= 16, 1 <= nchi <= 16.
- * Other arguments, ordering and error behaviour as sc_ivr_run; SC_IVR_EUNSUPPORTED when the grid is not equally spaced or too
- * long for the chirp-z stage.
+ * Other arguments, ordering and error behaviour as sc_ivr_run, except that this call ALWAYS synchronises the stream before it
+ * returns (with or without n_good_out); SC_IVR_EUNSUPPORTED when the grid is not equally spaced or too long for the chirp-z
+ * stage.
  */
 size_t sc_ivr_multi_workspace_bytes(const sc_ivr_ctx *ctx, long long ntraj, int k, int ncs, long long max_batch /*0 = 32768*/);
 sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double *weights, long long ntraj, const double *chis,

@@ -94,6 +94,8 @@ def lib():
     L.sc_ivr_set_timing.argtypes = [_vp, C.c_int]
     L.sc_ivr_last_timings.restype = C.c_int
     L.sc_ivr_last_timings.argtypes = [_vp, _dp]
+    L.sc_ivr_last_fallbacks.restype = C.c_longlong
+    L.sc_ivr_last_fallbacks.argtypes = [_vp]
     _lib = L
     return L
 
@@ -172,9 +174,7 @@ class ScIvr:
 
     def last_fallbacks(self):
         """Trajectory-steps of the last synchronising run that needed the pivoted eliminations (-1: not read back)."""
-        f = lib().sc_ivr_last_fallbacks
-        f.restype, f.argtypes = C.c_longlong, [_vp]
-        return int(f(self._h))
+        return int(lib().sc_ivr_last_fallbacks(self._h))
 
     def set_timing(self, on=True):
         lib().sc_ivr_set_timing(self._h, 1 if on else 0)

@@ -26,6 +26,15 @@ sc_ivr_status fail(sc_ivr_ctx *ctx, sc_ivr_status st, const char *fmt, ...) {
   return st;
 }
 
+// every entry point that launches work: the context's device (kernel attributes, coefficient buffers) must be current
+sc_ivr_status check_device(sc_ivr_ctx *ctx) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return fail(ctx, SC_IVR_ECUDA, "cannot query the current device");
+  if (dev != ctx->device)
+    return fail(ctx, SC_IVR_EINVAL, "context belongs to device %d but device %d is current", ctx->device, dev);
+  return SC_IVR_OK;
+}
+
 #define CU(call)                                                                                   \
   do {                                                                                             \
     cudaError_t e_ = (call);                                                                       \
@@ -197,8 +206,12 @@ struct StageTimer {
     if (!on) return;
     if (ctx->ev.size() < ctx->ev_used + 2) {
       cudaEvent_t a = nullptr, b = nullptr;
-      cudaEventCreate(&a);
-      cudaEventCreate(&b);
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {  // timing is a measurement aid: switch it off
+        if (a) cudaEventDestroy(a);
+        on = false;
+        ctx->timing = 0;
+        return;
+      }
       ctx->ev.push_back(a);
       ctx->ev.push_back(b);
     }
@@ -372,6 +385,7 @@ sc_ivr_status sc_ivr_run(sc_ivr_ctx *ctx, const double *p0q0, const double *weig
                          const double *E, int k, double *I_out, long long *n_good_out, void *workspace,
                          size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!p0q0 || !chi || !E || !I_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (ntraj < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "ntraj and k must be >= 1");
   if (((uintptr_t)workspace & 255) != 0) return fail(ctx, SC_IVR_EINVAL, "workspace must be 256-byte aligned");
@@ -494,6 +508,7 @@ sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double 
                               const double *E, int k, double *I_out, long long *n_good_out, void *workspace,
                               size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!p0q0 || !I_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (ntraj < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "ntraj and k must be >= 1");
   const size_t stg = sc_ivr_host_staging_bytes(ctx, ntraj, k);
@@ -505,11 +520,20 @@ sc_ivr_status sc_ivr_run_host(sc_ivr_ctx *ctx, const double *p0q0, const double 
   double *d_w = (double *)(ws + align_up(n_pq, 256));
   double *d_I = (double *)((char *)d_w + align_up(sizeof(double) * (size_t)ntraj, 256));
   CU(cudaMemcpyAsync(d_pq, p0q0, n_pq, cudaMemcpyHostToDevice, st));
-  if (weights) CU(cudaMemcpyAsync(d_w, weights, sizeof(double) * (size_t)ntraj, cudaMemcpyHostToDevice, st));
+  if (weights) {
+    const cudaError_t ce = cudaMemcpyAsync(d_w, weights, sizeof(double) * (size_t)ntraj, cudaMemcpyHostToDevice, st);
+    if (ce != cudaSuccess) {
+      cudaStreamSynchronize(st);  // the copy of p0q0 may still read the caller's pinned buffer
+      return fail(ctx, SC_IVR_ECUDA, "copy of the weights: %s", cudaGetErrorString(ce));
+    }
+  }
   long long ng = 0;
   sc_ivr_status rc = sc_ivr_run(ctx, d_pq, weights ? d_w : nullptr, ntraj, chi, E, k, d_I, &ng, ws + stg, workspace_bytes - stg, st);
   if (n_good_out) *n_good_out = ng;
-  if (rc != SC_IVR_OK && rc != SC_IVR_ENOGOOD) return rc;
+  if (rc != SC_IVR_OK && rc != SC_IVR_ENOGOOD) {
+    cudaStreamSynchronize(st);  // no copy from the caller's host buffers is left in flight when an error is returned
+    return rc;
+  }
   CU(cudaMemcpyAsync(I_out, d_I, sizeof(double) * (size_t)k, cudaMemcpyDeviceToHost, st));
   CU(cudaStreamSynchronize(st));
   return rc;
@@ -524,6 +548,7 @@ sc_ivr_status sc_ivr_propagate(sc_ivr_ctx *ctx, const double *p0q0, long long nt
                                double *pq_out, double *S_out, double *M_out, double *theta_out, unsigned char *good_out,
                                double *z_out, void *workspace, size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!p0q0) return fail(ctx, SC_IVR_EINVAL, "p0q0 is NULL");
   if (ntraj < 1 || nsteps_run < 0) return fail(ctx, SC_IVR_EINVAL, "ntraj must be >= 1 and nsteps_run >= 0");
   const bool need_raw = theta_out || z_out;
@@ -553,6 +578,7 @@ sc_ivr_status sc_ivr_propagate(sc_ivr_ctx *ctx, const double *p0q0, long long nt
 sc_ivr_status sc_ivr_eval_pes(sc_ivr_ctx *ctx, const double *q, long long n, double *V_out, double *g_out, double *H_out,
                               void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!q || !V_out || !g_out || !H_out) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (n < 1) return fail(ctx, SC_IVR_EINVAL, "n must be >= 1");
   if (ctx->F <= SCI_TPT_MAXF) {
@@ -577,6 +603,7 @@ size_t sc_ivr_fourier_workspace_bytes(const sc_ivr_ctx *ctx, long long n, int k)
 sc_ivr_status sc_ivr_fourier(sc_ivr_ctx *ctx, const double *zin, long long n, const double *E, int k, double *A_out,
                              void *workspace, size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!zin || !E || !A_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (n < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "n and k must be >= 1");
   if (workspace_bytes < sc_ivr_fourier_workspace_bytes(ctx, n, k)) return fail(ctx, SC_IVR_EINVAL, "workspace too small");
@@ -607,6 +634,7 @@ size_t sc_ivr_fourier_power_workspace_bytes(const sc_ivr_ctx *ctx, long long n, 
 sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *zin, long long n, const double *E, int k, double *P_out,
                                    void *workspace, size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!zin || !E || !P_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (n < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "n and k must be >= 1");
   if (workspace_bytes < sc_ivr_fourier_power_workspace_bytes(ctx, n, k)) return fail(ctx, SC_IVR_EINVAL, "workspace too small");
@@ -680,6 +708,7 @@ sc_ivr_status sc_ivr_run_multi(sc_ivr_ctx *ctx, const double *p0q0, const double
                                int ncs, const double *eps, int nchi, const double *E, int k, double *I_out,
                                long long *n_good_out, void *workspace, size_t workspace_bytes, void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
   if (!p0q0 || !chis || !eps || !E || !I_out || !workspace) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
   if (ntraj < 1 || k < 1) return fail(ctx, SC_IVR_EINVAL, "ntraj and k must be >= 1");
   if (ncs < 1 || ncs > 16 || nchi < 1 || nchi > 16) return fail(ctx, SC_IVR_EINVAL, "ncs and nchi must be in 1..16");

@@ -367,8 +367,8 @@ __global__ void __maxnreg__(SCI_ZREG) k_zassemble_rows(const double4 *__restrict
       for (int u = 0; u < SCI_ZU; u++) {
         const int cc = cb + u, c = c0 + cc;
         if (cc >= cn) break;
-        const double4 r = rec[u];
-        const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
+        double4 r = rec[u];
+        const double inv = unit_scale(r.z, r.w);
         const double x = r.z * inv, y = r.w * inv;
         double ur, ui;
         if (x >= 0.0) {
@@ -413,8 +413,8 @@ __global__ void __maxnreg__(128) k_overlap_phase(const double4 *__restrict__ raw
   if (j >= nb) return;
   double upr = 1.0, upi = 0.0;
   for (int c = 0; c <= nsteps; c++) {
-    const double4 r = raw[(long long)c * raw_stride + j];
-    const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
+    double4 r = raw[(long long)c * raw_stride + j];
+    const double inv = unit_scale(r.z, r.w);
     const double x = r.z * inv, y = r.w * inv;
     double ur, ui;
     if (x >= 0.0) {
@@ -510,13 +510,12 @@ cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, 
                                  const double *wg, int k, int kp, double *out, double2 *spec_out, int nblocks, int bsz,
                                  double2 *yscr, int grid, cudaStream_t st) {
   const size_t smem = sci_chirp_smem_bytes();
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_chirp_fft<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chirp_fft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_chirp_fft<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  {  // the attribute is per device and the call is cheap: set it on every launch (no process-wide flag)
+    cudaError_t e = cudaSuccess;
+    if (mode == 0) e = cudaFuncSetAttribute(k_chirp_fft<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    else if (mode == 1) e = cudaFuncSetAttribute(k_chirp_fft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    else e = cudaFuncSetAttribute(k_chirp_fft<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   if (mode == 0) {
     k_chirp_fft<0><<<grid, CT, smem, st>>>(x, xstride, n1, nrows, HpT, wg, k, kp, out, spec_out, nblocks, bsz, yscr);

@@ -132,3 +132,18 @@ cudaError_t sci_launch_rows_from_z(const double2 *z, long long n, int n1, const 
 cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, int n1, long long nrows, const double2 *HpT,
                                  const double *wg, int k, int kp, double *out, double2 *spec_out, int nblocks, int bsz,
                                  double2 *yscr, int grid, cudaStream_t st);
+
+#ifdef __CUDACC__
+// 1 / |D| for D = (re, im) without overflow or underflow of the squares: the determinant record carries an arbitrary positive
+// factor (the static elimination hands over det 2K times |prod 1/pivot|^2), so it is brought to unit scale by a power of two
+// taken from the larger component's exponent before it is squared (the oracle uses cabs)
+__device__ __forceinline__ double unit_scale(double &re, double &im) {
+  const int ex = (int)((max((unsigned)__double2hiint(re) & 0x7fffffffu, (unsigned)__double2hiint(im) & 0x7fffffffu) >> 20) & 0x7ffu);
+  if (ex > 0 && ex < 0x7fe) {
+    const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex)
+    re *= sc;
+    im *= sc;
+  }
+  return 1.0 / sqrt(fma(re, re, im * im));
+}
+#endif

@@ -23,8 +23,8 @@ __global__ void __launch_bounds__(128) k_zassemble(const double4 *__restrict__ r
   double theta = 0.0, arg_prev = 0.0;
   const double PI = 3.14159265358979323846;
   for (int c = 0; c <= nsteps; c++) {
-    const double4 r = raw[(long long)c * raw_stride + j];
-    const double inv = 1.0 / sqrt(fma(r.z, r.z, r.w * r.w));
+    double4 r = raw[(long long)c * raw_stride + j];
+    const double inv = unit_scale(r.z, r.w);
     const double x = r.z * inv, y = r.w * inv;
     double ur, ui;
     if (x >= 0.0) {
@@ -283,11 +283,9 @@ cudaError_t sci_launch_twiddle(const double *E_dev, int k, int kp, int rows, dou
 cudaError_t sci_launch_fourier(const double2 *z, long long zstride, long long zcols, int zrows, const double2 *W, int kp,
                                long long nb, const double *wg, double *partial, double2 *A_out, int k, cudaStream_t st) {
   const size_t smem = sizeof(double2) * STAGES * KC * (TJ + TI);
-  static bool attr_set = false;
-  if (!attr_set) {
+  {  // per device, cheap: set on every launch
     cudaError_t e = cudaFuncSetAttribute(k_fourier, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   dim3 grid(kp / TI, (unsigned)(zcols / TJ));
   k_fourier<<<grid, FTHREADS, smem, st>>>(z, zstride, zrows, W, kp, nb, wg, partial, A_out, k);

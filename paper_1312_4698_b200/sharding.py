@@ -18,6 +18,21 @@ def shard_bounds(ntraj: int, rank: int, world: int):
     return lo, lo + base + (1 if rank < rem else 0)
 
 
+def combine_shards(spectra, n_goods):
+    """The same re-weighting without a process group: spectra[r] (normalised by n_goods[r]) of every shard, in rank order.
+    Returns (I, n_good).  combine_spectra is this sum carried by one all-reduce."""
+    import torch
+
+    acc = torch.zeros_like(spectra[0])
+    n_good = 0
+    for I_r, n_r in zip(spectra, n_goods):  # fixed rank order
+        acc = acc + I_r * float(n_r)
+        n_good += int(n_r)
+    if n_good == 0:
+        return torch.zeros_like(spectra[0]), 0
+    return acc / float(n_good), n_good
+
+
 def combine_spectra(I_local, n_good_local: int, group=None):
     """All-reduce of (n_good_r * I_r, n_good_r): returns (I, n_good) of the whole job on every rank.
 

@@ -468,3 +468,32 @@ def test_full_size_sampled_trajectories(torch_cuda, B, oracle, cfg, ntraj, nstep
     If = If.cpu().numpy()
     assert rcf == 0 and ngf == ng and np.all(np.isfinite(If)) and np.all(If >= 0)
     assert np.all(If * ngf >= Io * ngo * (1 - 1e-9) - 1e-12 * Io.max() * ngo)
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_shards_of_a_real_run_recombine(torch_cuda, B, world):
+    """Rows e / f5 on one GPU: sc_ivr_run on the blocks shard_bounds gives each rank, one
+    block holding a poisoned trajectory so that its n_good differs, combined with the arithmetic of combine_spectra
+    (Eq. 11's 1 / n_good is per job), against the unsharded run."""
+    from paper_1312_4698_b200.sharding import combine_shards, combine_spectra, shard_bounds
+    torch = torch_cuda
+    w = inputs.make_config(4, ntraj=331, nsteps=300, k=200)
+    pq = w.p0q0.copy()
+    pq[0, 17] = np.nan  # lands in the first shard for world = 2 and 3
+    ctx = B.ScIvr.from_workload(w)
+    I_all, ng_all, rc = ctx.run(_dev(torch, pq), w.chi, w.E)
+    assert rc == 0 and ng_all == 330
+    parts, ngs = [], []
+    for r in range(world):
+        lo, hi = shard_bounds(w.ntraj, r, world)
+        I_r, ng_r, rc = ctx.run(_dev(torch, pq[:, lo:hi]), w.chi, w.E)
+        assert rc == 0
+        parts.append(I_r.clone())
+        ngs.append(ng_r)
+    assert sum(ngs) == ng_all and ngs[0] == shard_bounds(w.ntraj, 0, world)[1] - 1
+    I, ng = combine_shards(parts, ngs)
+    assert ng == ng_all
+    assert float((I - I_all).abs().max()) <= 1e-13 * float(I_all.max())
+    # the collective entry point with no process group is the one-shard case of the same sum
+    I1, ng1 = combine_spectra(I_all, ng_all)
+    assert ng1 == ng_all and float((I1 - I_all).abs().max()) <= 4e-16 * float(I_all.max())  # x n / n

@@ -7,7 +7,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_1312_4698_b200.sharding import combine_spectra, shard_bounds
+from paper_1312_4698_b200.sharding import combine_shards, combine_spectra, shard_bounds
 
 
 def _free_port():
@@ -59,3 +59,14 @@ def test_combine_single_process_no_group():
     assert ng == 5 and torch.equal(I, torch.tensor([1.0, 2.0], dtype=torch.float64))
     I, ng = combine_spectra(torch.tensor([1.0, 2.0], dtype=torch.float64), 0)
     assert ng == 0 and not I.any()
+
+
+def test_combine_shards_equals_the_collective_arithmetic():
+    rng = np.random.default_rng(1)
+    parts = [torch.from_numpy(rng.uniform(0, 1, 5)) for _ in range(3)]
+    ngs = [4, 0, 9]
+    I, ng = combine_shards(parts, ngs)
+    want = (parts[0] * 4 + parts[2] * 9) / 13
+    assert ng == 13 and float((I - want).abs().max()) < 1e-15
+    I0, ng0 = combine_shards(parts, [0, 0, 0])
+    assert ng0 == 0 and float(I0.abs().max()) == 0.0
