@@ -34,29 +34,49 @@ UNIT = "trajectory-steps/s"
 # The guides give no FP64 unit count; 64 lanes/SM/clk is what this library's own DFMA/DMMA probe
 # measures (37.2 TFLOP/s with mma.sync m8n8k4 f64 at 1965 MHz) - the probe value is reported beside it.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at the bench configuration,
-# from the ncu --set full capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = {"propagate": 16974059640, "fourier": None}  # profiles/r01c_kernelA_full_config4.md
-CHIRP_L = 8192  # circular convolution length of the chirp-z Fourier stage (csrc/common.cuh SCI_CHIRP_L)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel A from one `ncu --set full` capture of the bench command,
+# keyed by (workload, ntraj, nsteps, det_stride); the capture is summarised in the profiles/ file named beside it.  Any
+# other configuration reports null.
+NCU_TRAFFIC_BYTES = {
+    ("config4_qff_ch4", 131072, 4000, 1): (None, "profiles/r02_kernelA_ncu_config4.md"),
+}
+CHIRP_L = 8192          # circular convolution length of the chirp-z Fourier stage (csrc/common.cuh SCI_CHIRP_L)
+CHIRP_MIN_BLOCK = 1024  # csrc/common.cuh SCI_CHIRP_MIN_BLOCK
+CHIRP_MAX_BLOCKS = 16   # csrc/common.cuh SCI_CHIRP_MAX_BLOCKS
+# SURVEY.md 8d, complex determinant column (the survey rounds its own count; the formula below is used for other F)
+SURVEY_CDET = {1: 10, 3: 95, 6: 615, 9: 1980}
 
 
-def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False, nsteps: int = 4000, chirp: bool = True):
-    """Algorithmic flop per trajectory-step (SURVEY.md 8d table, 1 FMA = 2 flop).  Fourier stage: the direct sum of
-    Eq. 11 is 8k per trajectory-step; on an equally spaced grid the library evaluates it as a chirp-z transform
-    (two FFTs of length 8192 per trajectory), whose own count 2 * 5 L log2 L / (nsteps + 1) is what is credited."""
-    pes = 60 if morse else 2 * (F * F * (F + 1) // 2 + 2 * F * F + F * (F - 1) + 6 * F)
+def chirp_blocks(nsteps: int, k: int):
+    """Mirror of the library's chirp_plan (csrc/api.cu): number of chirp-z blocks, 0 = direct sum."""
+    if nsteps + k <= CHIRP_L:
+        return 1
+    bsz = CHIRP_L + 1 - k
+    if bsz < CHIRP_MIN_BLOCK:
+        return 0
+    nb = -(-(nsteps + 1) // bsz)
+    return nb if nb <= CHIRP_MAX_BLOCKS else 0
+
+
+def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False, nsteps: int = 4000, nblocks: int = 1):
+    """Algorithmic flop per trajectory-step: SURVEY.md 8d's table (1 FMA = 2 flop), column by column; F = 9 QFF gives
+    1386 + 150 + 3888 + 486 + 1980 = 7890, + 3570 with the det M check at every step = 11460.  Fourier stage: the direct
+    sum of Eq. 11 is 8k per trajectory-step; on an equally spaced grid the library evaluates it as a chirp-z transform
+    (two FFTs of length 8192 per trajectory and block), whose own count 2 * 5 L log2 L * nblocks / (nsteps + 1) is what is
+    credited; nblocks = 0 means the direct sum."""
+    pes = 60 * F if morse else 2 * (F * F * (F + 1) // 2 + 2 * F * F + F * (F - 1) + 6 * F)
     step = 16 * F + 6
     mono = 2 * (2 * F ** 3 + 6 * F ** 2)
     kmat = 6 * F * F
-    cdet = 8 * (F - 1) * F * (2 * F - 1) // 6 + 6 * F * (F - 1) // 2 + 16 * F
+    cdet = SURVEY_CDET.get(F, 8 * (F - 1) * F * (2 * F - 1) // 6 + 6 * F * (F - 1) // 2 + 16 * F)
     # SURVEY's table also lists ~150 flop-equivalents of transcendentals (exp, sincos, sqrt branch of z_c): this build does
     # them in the z assembly kernel, not in kernel A, so they are NOT credited to kernel A's roofline fraction
     a_total = pes + step + mono + kmat + cdet
     n = 2 * F
-    check = 2 * ((n - 1) * n * (2 * n - 1) // 6) + n * (n - 1) // 2 + 12 * n
+    check = 2 * ((n - 1) * n * (2 * n - 1) // 6)  # SURVEY 8d "+det M check": the FMAs of the real 2F x 2F elimination
     if det_every_step:
         a_total += check
-    fourier = 2 * 5 * CHIRP_L * math.log2(CHIRP_L) / (nsteps + 1) if chirp else 8 * k
+    fourier = 2 * 5 * CHIRP_L * math.log2(CHIRP_L) * nblocks / (nsteps + 1) if nblocks > 0 else 8 * k
     return dict(propagate=a_total, fourier=fourier)
 
 
@@ -103,7 +123,25 @@ def cpu_oracle_sample(w, ntraj_sample: int, det_stride: int):
                 sample=f"first {ws.ntraj} trajectories of {w.name}, {w.nsteps} steps, {w.k} energies, det_stride={det_stride}: {dt:.1f} s"), dt
 
 
-def make_workload(config: int, rank: int, ntraj: int | None, nsteps: int | None = None, k: int | None = None):
+def single_thread_oracle(args, ntraj_sample: int):
+    """The paper's CPU numbers are single-thread: the same oracle with OMP_NUM_THREADS=1, in a process of its
+    own (the OpenMP runtime reads the variable once), on a smaller sample of the same workload."""
+    cmd = [sys.executable, os.path.abspath(__file__), "--impl", "reference", "--config", str(args.config), "--steps", "1", "--warmup", "0",
+           "--ref-sample", str(ntraj_sample), "--det-stride", str(args.det_stride)]
+    for flag, v in (("--ntraj", args.ntraj), ("--nsteps", args.nsteps), ("--k", args.k), ("--morse", args.morse or None)):
+        if v is not None:
+            cmd += [flag, str(v)]
+    try:
+        out = subprocess.run(cmd, env=dict(os.environ, OMP_NUM_THREADS="1", RANK="0", WORLD_SIZE="1"), capture_output=True, text=True, timeout=900)
+        d = json.loads(out.stdout.strip().splitlines()[-1])
+        return dict(value=d["value"], unit=UNIT, cores=d["cpu_baseline"]["cores"], sample=d["cpu_baseline"]["sample"])
+    except Exception as ex:  # a reported baseline only
+        return dict(error=str(ex)[:200])
+
+
+def make_workload(config: int, rank: int, ntraj: int | None, nsteps: int | None = None, k: int | None = None, morse: int = 0):
+    if morse:  # PAPER.md:204-206, Fig. 6: F uncoupled Morse oscillators, "the same number of trajectories"
+        return inputs.make_uncoupled_morse(morse, ntraj or 65536, nsteps or 4000, k or 4000, seed=11 + rank)
     if rank == 0 and config != 5:
         return inputs.make_config(config, ntraj=ntraj, nsteps=nsteps, k=k)
     # rank r > 0 (weak scaling): block r of config 5's 2^20-row draw on config 4's surface, same size as rank 0's
@@ -117,7 +155,7 @@ def make_workload(config: int, rank: int, ntraj: int | None, nsteps: int | None 
 def run_reference(args, rank):
     if rank != 0:
         return
-    w = make_workload(args.config, 0, args.ntraj, args.nsteps, args.k)
+    w = make_workload(args.config, 0, args.ntraj, args.nsteps, args.k, args.morse)
     times = []
     for i in range(args.warmup + args.steps):
         cb, dt = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
@@ -146,11 +184,17 @@ def main():
     ap.add_argument("--nsteps", type=int, default=None)
     ap.add_argument("--k", type=int, default=None)
     ap.add_argument("--det-stride", type=int, default=1)
-    ap.add_argument("--ref-sample", type=int, default=1024)
+    ap.add_argument("--ref-sample", type=int, default=None,
+                    help="trajectories of the oracle sample; default 2048 (BASELINE.md section 3), shrunk in the reference arm so that "
+                         "steps + warmup samples end within a few minutes")
+    ap.add_argument("--ref-sample-1t", type=int, default=64, help="trajectories of the single-thread oracle sample; 0 = skip")
+    ap.add_argument("--morse", type=int, default=0, help="F uncoupled Morse oscillators instead of a BASELINE config (row f3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nchi", type=int, default=0,
                     help="measure sc_ivr_run_multi with this many reference states (row f4) instead of sc_ivr_run; short JSON line")
     args = ap.parse_args()
+    if args.ref_sample is None:
+        args.ref_sample = 2048 if args.impl == "ours" else max(256, 2048 // max(1, (args.steps + args.warmup + 5) // 6))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -169,7 +213,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     B.lib()
 
-    w = make_workload(args.config, rank, args.ntraj, args.nsteps, args.k)
+    w = make_workload(args.config, rank, args.ntraj, args.nsteps, args.k, args.morse)
     ctx = B.ScIvr.from_workload(w, det_stride=args.det_stride)
     ctx.set_timing(True)
     d_pq = torch.from_numpy(w.p0q0).cuda()
@@ -250,9 +294,10 @@ def main():
     e2e_value = units / (e2e_ms * 1e-3)
 
     if rank == 0:
-        chirp = (w.nsteps + w.k <= CHIRP_L)  # inputs.energy_grid is equally spaced
-        fm = flop_model(w.F, w.k, args.det_stride == 1, morse=(w.pes_kind != inputs.PES_QFF), nsteps=w.nsteps, chirp=chirp)
-        kname = {"propagate": "k_propagate_tpt" if w.F <= 3 else "k_propagate", "fourier": "k_chirp_fft" if chirp else "k_fourier"}
+        nblk = chirp_blocks(w.nsteps, w.k)  # inputs.energy_grid is equally spaced: the library takes the chirp-z path when it can
+        chirp = nblk > 0
+        fm = flop_model(w.F, w.k, args.det_stride == 1, morse=(w.pes_kind != inputs.PES_QFF), nsteps=w.nsteps, nblocks=nblk)
+        kname = {"propagate": "k_propagate_tpt" if w.F <= 3 else "k_propagate_cml", "fourier": "k_chirp_fft" if chirp else "k_fourier"}
         dom = "fourier" if stage["fourier_ms"] >= stage["propagate_ms"] else "propagate"
         dom_ms = stage[dom + "_ms"]
         flops_per_launch = fm[dom] * w.ntraj * w.nsteps  # one launch per run when the workload is a single batch
@@ -266,6 +311,10 @@ def main():
         cpu = None
         if not args.no_cpu_baseline:
             cpu, _ = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
+            if args.ref_sample_1t > 0:
+                cpu["single_thread"] = single_thread_oracle(args, args.ref_sample_1t)
+        traffic, traffic_src = NCU_TRAFFIC_BYTES.get((w.name, w.ntraj, w.nsteps, args.det_stride), (None, None)) if dom == "propagate" else (None, None)
+        dfma = probe.get("dfma_tflops")
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -279,8 +328,10 @@ def main():
                     "d2h_bytes_per_step": int(w.k * 8 + 8)},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "kernel": kname[dom], "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES[dom],
-                         "peak_source": "148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md); this run's FP64 probes alongside",
+                         "frac": achieved / FP64_PEAK_TFLOPS, "frac_vs_dfma_probe": (achieved / dfma) if dfma else None,
+                         "traffic": traffic, "traffic_source": traffic_src,
+                         "peak_source": "nominal: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md; MEASURED_PEAKS.json has no FP64 entry); "
+                                        "frac_vs_dfma_probe divides by this run's measured DFMA rate instead",
                          "flop_per_trajectory_step": fm[dom], "probe": probe,
                          "other_kernel": {"kernel": kname[other], "achieved": other_tf, "frac": other_tf / FP64_PEAK_TFLOPS,
                                           "flop_per_trajectory_step": fm[other]}},
