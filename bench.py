@@ -38,7 +38,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # keyed by (workload, ntraj, nsteps, det_stride); the capture is summarised in the profiles/ file named beside it.  Any
 # other configuration reports null.
 NCU_TRAFFIC_BYTES = {
-    ("config4_qff_ch4", 131072, 4000, 1): (None, "profiles/r02_kernelA_ncu_config4.md"),
+    ("config4_qff_ch4", 131072, 4000, 1): (16759154000 + 121386496, "profiles/r02_kernelA_ncu_config4.md"),  # write + read
 }
 CHIRP_L = 8192          # circular convolution length of the chirp-z Fourier stage (csrc/common.cuh SCI_CHIRP_L)
 CHIRP_MIN_BLOCK = 1024  # csrc/common.cuh SCI_CHIRP_MIN_BLOCK
