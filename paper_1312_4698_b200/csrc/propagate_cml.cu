@@ -149,7 +149,7 @@ struct Cml {
 #ifndef SCI_CML_ST_W
 #define SCI_CML_ST_W 128
 #endif
-template <int ND, int WMAX>
+template <int ND, int WMAX, bool WAIT = true>
 __device__ __forceinline__ void tmem_st_f64_w(uint32_t taddr, const double (&d)[ND]) {
   uint32_t v[2 * ND];
 #pragma unroll
@@ -158,7 +158,7 @@ __device__ __forceinline__ void tmem_st_f64_w(uint32_t taddr, const double (&d)[
     v[2 * i + 1] = (uint32_t)__double2hiint(d[i]);
   }
   tmem_st_issue<2 * ND, 0, WMAX>(taddr, v);
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  if (WAIT) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
 // one column of M from / to the lane's tensor memory: rows 0..F-1 (dP) and F..2F-1 (dQ) live in different halves
@@ -369,8 +369,8 @@ __device__ __forceinline__ void pass_cml(uint32_t tm, const LaneAddr &A, const P
 #pragma unroll
     for (int e = 0; e < C * F; e += 2)
       sts2(hmh + X::hm(e), HM[e / F][e % F], (e + 1 < C * F) ? HM[(e + 1) / F][(e + 1) % F] : 0.0);
+    tmem_st_f64_w<C * F, SCI_CML_ST_W, false>(tmh + X::TH * 2, sq);
     tmem_st_f64_w<C * F, SCI_CML_ST_W>(tmh, sp);
-    tmem_st_f64_w<C * F, SCI_CML_ST_W>(tmh + X::TH * 2, sq);
   }
 }
 
