@@ -112,12 +112,12 @@ class ClockSampler(threading.Thread):
                     samples=len(sm))
 
 
-def cpu_oracle_sample(w, ntraj_sample: int, det_stride: int):
+def cpu_oracle_sample(w, ntraj_sample: int, det_stride: int, integrator: int = 0):
     """The oracle as it stands, on the first ntraj_sample trajectories of the workload (full time and energy grid)."""
     from oracle import capi
     ws = w.prefix(min(ntraj_sample, w.ntraj))
     t0 = time.perf_counter()
-    capi.run_workload(ws, det_stride=det_stride)
+    capi.run_workload(ws, det_stride=det_stride, integrator=integrator)
     dt = time.perf_counter() - t0
     return dict(value=ws.ntraj * w.nsteps / dt, unit=UNIT, cores=capi.num_threads(), kind="oracle",
                 sample=f"first {ws.ntraj} trajectories of {w.name}, {w.nsteps} steps, {w.k} energies, det_stride={det_stride}: {dt:.1f} s"), dt
@@ -128,7 +128,8 @@ def single_thread_oracle(args, ntraj_sample: int):
     own (the OpenMP runtime reads the variable once), on a smaller sample of the same workload."""
     cmd = [sys.executable, os.path.abspath(__file__), "--impl", "reference", "--config", str(args.config), "--steps", "1", "--warmup", "0",
            "--ref-sample", str(ntraj_sample), "--det-stride", str(args.det_stride)]
-    for flag, v in (("--ntraj", args.ntraj), ("--nsteps", args.nsteps), ("--k", args.k), ("--morse", args.morse or None)):
+    for flag, v in (("--ntraj", args.ntraj), ("--nsteps", args.nsteps), ("--k", args.k), ("--morse", args.morse or None),
+                    ("--integrator", args.integrator or None)):
         if v is not None:
             cmd += [flag, str(v)]
     try:
@@ -158,7 +159,7 @@ def run_reference(args, rank):
     w = make_workload(args.config, 0, args.ntraj, args.nsteps, args.k, args.morse)
     times = []
     for i in range(args.warmup + args.steps):
-        cb, dt = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
+        cb, dt = cpu_oracle_sample(w, args.ref_sample, args.det_stride, args.integrator)
         if i >= args.warmup:
             times.append(dt)
     n = min(args.ref_sample, w.ntraj)
@@ -188,6 +189,9 @@ def main():
                     help="trajectories of the oracle sample; default 2048 (BASELINE.md section 3), shrunk in the reference arm so that "
                          "steps + warmup samples end within a few minutes")
     ap.add_argument("--ref-sample-1t", type=int, default=64, help="trajectories of the single-thread oracle sample; 0 = skip")
+    ap.add_argument("--integrator", type=int, default=0, choices=[0, 1],
+                    help="0 = velocity-Verlet (BASELINE.json), 1 = 4-stage 4th-order symplectic scheme (the paper's, PAPER.md:109; row f2): "
+                         "four evaluation points per time step, the flop model is scaled accordingly")
     ap.add_argument("--morse", type=int, default=0, help="F uncoupled Morse oscillators instead of a BASELINE config (row f3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nchi", type=int, default=0,
@@ -214,7 +218,7 @@ def main():
     B.lib()
 
     w = make_workload(args.config, rank, args.ntraj, args.nsteps, args.k, args.morse)
-    ctx = B.ScIvr.from_workload(w, det_stride=args.det_stride)
+    ctx = B.ScIvr.from_workload(w, det_stride=args.det_stride, integrator=args.integrator)
     ctx.set_timing(True)
     d_pq = torch.from_numpy(w.p0q0).cuda()
     ws_bytes = ctx.workspace_bytes(w.ntraj, w.k) + ctx.host_staging_bytes(w.ntraj, w.k)
@@ -297,6 +301,11 @@ def main():
         nblk = chirp_blocks(w.nsteps, w.k)  # inputs.energy_grid is equally spaced: the library takes the chirp-z path when it can
         chirp = nblk > 0
         fm = flop_model(w.F, w.k, args.det_stride == 1, morse=(w.pes_kind != inputs.PES_QFF), nsteps=w.nsteps, nblocks=nblk)
+        if args.integrator == 1:  # PES, step and monodromy columns of SURVEY 8d are per evaluation point: four per time step
+            f1 = flop_model(w.F, w.k, False, morse=(w.pes_kind != inputs.PES_QFF), nsteps=w.nsteps, nblocks=nblk)["propagate"]
+            F_ = w.F
+            per_point = f1 - 6 * F_ * F_ - SURVEY_CDET.get(F_, 8 * (F_ - 1) * F_ * (2 * F_ - 1) // 6 + 6 * F_ * (F_ - 1) // 2 + 16 * F_)
+            fm["propagate"] += 3 * per_point
         kname = {"propagate": "k_propagate_tpt" if w.F <= 3 else "k_propagate_cml", "fourier": "k_chirp_fft" if chirp else "k_fourier"}
         dom = "fourier" if stage["fourier_ms"] >= stage["propagate_ms"] else "propagate"
         dom_ms = stage[dom + "_ms"]
@@ -310,7 +319,7 @@ def main():
             probe = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline:
-            cpu, _ = cpu_oracle_sample(w, args.ref_sample, args.det_stride)
+            cpu, _ = cpu_oracle_sample(w, args.ref_sample, args.det_stride, args.integrator)
             if args.ref_sample_1t > 0:
                 cpu["single_thread"] = single_thread_oracle(args, args.ref_sample_1t)
         traffic, traffic_src = NCU_TRAFFIC_BYTES.get((w.name, w.ntraj, w.nsteps, args.det_stride), (None, None)) if dom == "propagate" else (None, None)
@@ -320,7 +329,7 @@ def main():
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "F": w.F, "ntraj_per_gpu": w.ntraj, "nsteps": w.nsteps, "k": w.k, "dt": w.dt,
-                       "det_stride": args.det_stride, "integrator": "velocity-verlet",
+                       "det_stride": args.det_stride, "integrator": "velocity-verlet" if args.integrator == 0 else "4-stage 4th-order (McLachlan-Atela)",
                        "l2": "working set per step (raw 32 B + z 16 B per trajectory-step) exceeds L2 by >100x; no flush needed",
                        "parallelism": f"trajectory shards x{world}, one all-reduce of k+1 doubles" if world > 1 else "single GPU"},
             "clocks": clocks,
