@@ -9,19 +9,26 @@
 // Where the state lives (per SM: one CTA of 8 warps):
 //   tensor memory   the lane's 2 C columns of M (4 C F doubles), exactly the matrix M(c) of the last integer time c:
 //                   TMEM is used as lane-private scratch through tcgen05.ld / tcgen05.st (32x32b), two warps per
-//                   32-lane quadrant, 128 doubles per lane each
-//   registers       the working copies of the two eliminations (a5: det 2K, complex F x F; a7: det M, real 2F x 2F)
-//   shared memory   per trajectory: Q exchange, Hessian entries, the pivot columns of the running elimination steps;
-//                   per lane: H dQ of the last evaluation point (used twice: closing kick before the snapshot, opening
-//                   kick after it)
+//                   32-lane quadrant, 128 doubles per lane each; layout [dP rows | dQ rows][column][F]
+//   registers       the working copies of the two eliminations (a5: det 2K, complex F x F; a7: det M, real 2F x 2F, in two
+//                   row halves) and of the pass
+//   shared memory   per trajectory: Q exchange, Hessian entries, cubic gradient terms of the PES; per lane: H dQ of the
+//                   last evaluation point (used twice: closing kick before the snapshot, opening kick after it)
+//   warp shuffles   the pivot columns of the eliminations (owner lane -> the L lanes of the trajectory): no shared memory,
+//                   no barrier in the snapshot
 //
 // Per time step (velocity-Verlet; the general "kick b_s, drift a_s" composition is a table of evaluation points):
 //   snapshot  M-LU and K-LU from the TMEM state (static pivot order with look-ahead, monitored multipliers, pivoted
-//             fallback), record (ln|<chi|pq>|, S + arg<chi|pq>, det 2K), flag |det M - 1| <= tol
+//             fallback, which also confirms every rejection), record (ln|<chi|pq>|, S + arg<chi|pq>, det 2K), flag
+//             |det M - 1| <= tol
 //   pass      scalars kick/drift; PES at the new Q (gradient, Hessian -> shared memory); per column: opening kick with
 //             the parked H dQ, drift, new H dQ, closing kick, store to TMEM, park H dQ
 //
 // Everything runs in reduced coordinates Q = sqrt(gamma) q, P = p / sqrt(gamma): 2K = (M_qq + M_pp) + i (M_pq - M_qp).
+//
+// This file is compiled once per row (F, L) of cml_table.h (-DSCI_CML_INST_F, -DSCI_CML_INST_L: the kernels) and once without
+// them (the dispatcher at the end).  Measurements, the instruction mix and the variants that were tried and dropped:
+// profiles/r02_kernelA_ncu_config4.md; design: DESIGN.md section 3.
 #include "common.cuh"
 #include "tmem_ldst.cuh"
 
