@@ -73,8 +73,10 @@ typedef struct {
   int integrator;  /* 0 = velocity-Verlet (default), 1 = 4-stage 4th-order symplectic */
   double lu_growth_max; /* the two determinants are eliminated in a fixed pivot order while every multiplier of det K
                            stays below lu_growth_max and every multiplier of det M below lu_growth_max^2; a step that
-                           exceeds them is repeated with pivoting.  0 = default 1e4;
-                           < 0 = always use the pivoted eliminations (testing) */
+                           exceeds them is repeated with pivoting, and so is the first step at
+                           which the fixed order finds |det M - 1| > det_tol: a trajectory is only rejected by the pivoted
+                           elimination.  0 = default 1e4; < 0 = always use the pivoted eliminations
+                           (testing) */
   int fourier_mode;     /* 0 = automatic: an equally spaced energy grid with k <= 7169 and at most 16
                            blocks of 8193 - k time samples takes the chirp-z (FFT) evaluation of the sum of Eq. 11,
                            anything else the direct sum; 1 = always the direct sum */
@@ -211,7 +213,8 @@ sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *z, long long n
 sc_ivr_status sc_ivr_fp64_probe(int mode, int iters, double *flops_out, double *ms_out);
 /* Number of trajectory-steps of the most recent sc_ivr_run with n_good_out != NULL (or sc_ivr_run_host) on ctx whose
  * determinants were repeated with the pivoted eliminations because a multiplier of the fixed-order elimination exceeded
- * lu_growth_max; -1 when that run did not read it back.  Statistics only. */
+ * lu_growth_max or because the fixed order was about to reject the trajectory; -1 when that run did not read it back.
+ * Statistics only. */
 long long sc_ivr_last_fallbacks(const sc_ivr_ctx *ctx);
 void sc_ivr_set_timing(sc_ivr_ctx *ctx, int on);
 sc_ivr_status sc_ivr_last_timings(sc_ivr_ctx *ctx, double out[6]);
