@@ -2,7 +2,7 @@
 // The whole state (2F + 4F^2 + 1 doubles = 43 at F = 3), H dQ and the working copies of both eliminations fit the
 // register file of one thread, so nothing is exchanged between lanes: no shared memory, no shuffles.  The reduced PES
 // constants are kernel parameters, i.e. warp-uniform constant-bank operands of the FMAs (no load instructions).
-// Same arithmetic as the lane-distributed kernel (propagate.cu): reduced coordinates, generic kick/drift stages,
+// Same arithmetic as the lane-distributed kernels (propagate_cml.cu): reduced coordinates, generic kick/drift stages,
 // fixed-order eliminations with a monitored multiplier growth and a pivoted fallback (here a plain loop over local
 // arrays, executed by the rare thread that needs it).
 #include "common.cuh"

@@ -275,7 +275,7 @@ def test_fallback_statistics(torch_cuda, B, cfg, ntraj):
 @pytest.mark.parametrize("F", list(range(1, 13)))
 @pytest.mark.parametrize("integ", [0, 1], ids=["verlet", "fourth_order"])
 def test_run_every_supported_F(torch_cuda, B, oracle, F, integ):
-    """The whole path for every F the library instantiates (thread-per-trajectory kernels F <= 3, F lanes per trajectory
+    """The whole path for every F the library instantiates (thread-per-trajectory kernels F <= 3, C modes per lane
     above), both integrators, random couplings, ragged sizes: I(E) against the oracle."""
     torch = torch_cuda
     w = inputs.make_uncoupled_morse(1, 70, 400, 96, seed=101) if F == 1 else inputs.make_random_qff(F, 40 + 3 * F, 400, 96, seed=101 + F)
