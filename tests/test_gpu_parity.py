@@ -91,6 +91,23 @@ def test_propagate_parity_1000_steps(torch_cuda, B, oracle, w):
     assert np.max(np.abs(z - r["z"])) < 1e-9
 
 
+@pytest.mark.parametrize("cfg,ntraj", [(4, 11839), (4, 11840), (4, 11850), (4, 12681), (3, 18944), (3, 18961)])
+def test_propagate_launch_shape_seams(torch_cuda, B, oracle, cfg, ntraj):
+    """Kernel A's launch shape (whole rounds of full CTAs + one evenly spread last round, launch_prop_cml) at its seams: one
+    trajectory short of a round of 148 CTAs, exactly one round, a last round of one warp, of one warp per SM + a few; every
+    trajectory's (p, q, S), flag and determinant phase against the oracle after a short run."""
+    torch = torch_cuda
+    w = inputs.make_config(cfg, ntraj=ntraj, nsteps=40, k=16)
+    ctx = B.ScIvr.from_workload(w)
+    o = ctx.propagate(_dev(torch, w.p0q0), w.nsteps, chi=w.chi, want_M=False)
+    r = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, w.p0q0, w.chi, want_M=False)
+    pq = o["pq"].cpu().numpy()
+    assert np.max(np.abs(pq - r["pq"]) / np.maximum(np.abs(r["pq"]), 1.0)) < 1e-11
+    assert np.max(np.abs(o["S"].cpu().numpy() - r["S"])) < 1e-10
+    assert np.max(np.abs(o["theta"].cpu().numpy() - r["theta"])) < 1e-9
+    assert np.array_equal(o["good"].cpu().numpy(), r["good"]) and r["good"].all()
+
+
 def test_propagate_fourth_order_and_stride(torch_cuda, B, oracle):
     """The 4-stage scheme and det_stride > 1 follow the oracle too."""
     torch = torch_cuda
