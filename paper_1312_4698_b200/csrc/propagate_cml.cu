@@ -88,7 +88,11 @@ __device__ __forceinline__ void sts2(uint32_t a, double x, double y) {
 // value of v on lane src (every lane of the warp executes this).  One 64-bit broadcast costs two SHFL = one cycle of
 // the SM's shared-memory data pipe, against 2 (LDS.64) + 1.3 (owner's STS.64) + a warp barrier through shared memory
 // (ncu: l1tex__data_pipe_lsu_wavefronts_mem_shared, profiles/r02b)
-__device__ __forceinline__ double bcast(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+template <int L>
+__device__ __forceinline__ double bcast(double v, int src) {
+  if (L == 1) return v;  // one lane per trajectory: the owner is the lane itself
+  return __shfl_sync(0xffffffffu, v, src);
+}
 
 // Optional barriers that keep the warps of a CTA in step (SCI_CML_SYNC = 1: one CTA barrier per time step; 6: the warps 4..
 // run half a time step behind the warps 0..3; 7: both).  Measured on config 4 (profiles/r02): none of them pays once the
@@ -406,8 +410,8 @@ struct KStep {
                                               double &ri, double (&pr)[F], double (&pi)[F]) {
 #pragma unroll
     for (int i = j; i < F; i++) {
-      pr[i] = bcast(Kr[s][i], src);
-      pi[i] = bcast(Ki[s][i], src);
+      pr[i] = bcast<L>(Kr[s][i], src);
+      pi[i] = bcast<L>(Ki[s][i], src);
     }
     const double rn = rcp_nr2(fma(pr[j], pr[j], pi[j] * pi[j]));
     rr = pr[j] * rn;
@@ -451,7 +455,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
     }
     double pc[F];
 #pragma unroll
-    for (int i = 0; i < F; i++) pc[i] = bcast(W[0][i], A.g0);
+    for (int i = 0; i < F; i++) pc[i] = bcast<L>(W[0][i], A.g0);
     double r = rcp_nr2(pc[0]);
 #pragma unroll
     for (int k = 0; k < F; k++) {
@@ -464,7 +468,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
 #pragma unroll
         for (int i = k + 1; i < F; i++) W[sn][i] = fma(-m[sn][k], pc[i], W[sn][i]);
 #pragma unroll
-        for (int i = k + 1; i < F; i++) pn[i] = bcast(W[sn][i], A.g0 + ((k + 1) % L) * G);
+        for (int i = k + 1; i < F; i++) pn[i] = bcast<L>(W[sn][i], A.g0 + ((k + 1) % L) * G);
         rn = rcp_nr2(pn[k + 1]);
       }
 #pragma unroll
@@ -496,7 +500,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
   {
     double pc[F];
 #pragma unroll
-    for (int i = 0; i < F; i++) pc[i] = bcast(W[0][i], A.g0);
+    for (int i = 0; i < F; i++) pc[i] = bcast<L>(W[0][i], A.g0);
 #pragma unroll
     for (int k = 0; k < F; k++) {
       const int sn = (k + 1 < F) ? (k + 1) / L : -1;
@@ -505,7 +509,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
 #pragma unroll
         for (int i = 0; i < F; i++) W[sn][i] = fma(-m[sn][k], pc[i], W[sn][i]);
 #pragma unroll
-        for (int i = 0; i < F; i++) pn[i] = bcast(W[sn][i], A.g0 + ((k + 1) % L) * G);
+        for (int i = 0; i < F; i++) pn[i] = bcast<L>(W[sn][i], A.g0 + ((k + 1) % L) * G);
       }
 #pragma unroll
       for (int s = 0; s < NS; s++) {
@@ -541,7 +545,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
   double rr = 1.0, ri = 0.0, pr[F], pi[F];
   if (F > 1) {
 #pragma unroll
-    for (int i = 0; i < F; i++) pc[i] = bcast(W[C][i], A.g0);
+    for (int i = 0; i < F; i++) pc[i] = bcast<L>(W[C][i], A.g0);
     r = rcp_nr2(pc[0]);
     KStep<F, L>::cast(0, 0, A.g0, Kr, Ki, rr, ri, pr, pi);
   }
@@ -564,7 +568,7 @@ __device__ __forceinline__ void lu_mk_cml(uint32_t tm, const LaneAddr &A, int l,
 #pragma unroll
         for (int i = j + 1; i < F; i++) W[C + sn][i] = fma(-mm, pc[i], W[C + sn][i]);
 #pragma unroll
-        for (int i = j + 1; i < F; i++) pn[i] = bcast(W[C + sn][i], src);
+        for (int i = j + 1; i < F; i++) pn[i] = bcast<L>(W[C + sn][i], src);
         rn = rcp_nr2(pn[j + 1]);
       }
       KStep<F, L>::upd(j, sn, l, Kr, Ki, rr, ri, pr, pi, gk);
