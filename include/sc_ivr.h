@@ -192,6 +192,35 @@ sc_ivr_status sc_ivr_fourier(sc_ivr_ctx *ctx, const double *z, long long n, cons
                              double *A_out, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
+ * The same sum (Eq. 11; the kernels of sc_ivr_fourier) for callers that CANNOT ALLOCATE device memory and so
+ * have no workspace to pass: a plug-in inside a program whose own pool took all of HBM at start-up (any later cudaMalloc
+ * fails there), a step in a latency-bound loop (cudaMalloc / cudaFree lock the driver and synchronise the device for an
+ * unbounded time), a process whose device-memory budget is fixed and spent.  The scratch (zero-padded copy of z + twiddle
+ * table) is a static array of SC_IVR_STATIC_SCRATCH_BYTES inside the library's device image; every GPU that loads the
+ * library's kernels holds it until the process exits.  The call needs no context, performs no cudaMalloc / cudaFree /
+ * cudaMemcpy and calls nothing that allocates.
+ *   z      DEVICE [nsteps+1][n][2] (time-major)      E      DEVICE [k] (not HOST: there is nowhere to stage a copy)
+ *   A_out  DEVICE [n][k][2], overwritten              dt     any finite value; nsteps >= 0
+ * Limit: sc_ivr_fourier_static_scratch_bytes(n, nsteps, k) = 16 ceil16(nsteps+1) (ceil128(n) + ceil64(k)) bytes (each term
+ * rounded to 256) must be <= SC_IVR_STATIC_SCRATCH_BYTES, e.g. n <= 128 trajectories x 1001 time samples x 896 energies;
+ * larger sizes are rejected with SC_IVR_EINVAL and a message that names both numbers (split the call over trajectories or
+ * energies, the sum is independent in both).  The size query returns 0 for arguments that are out of range.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, once per device, with that device
+ * current; thread-safe).  Make this first call outside any stream capture.  Later calls only launch kernels on cuda_stream.
+ * Sharing: there is ONE array per device.  Every call overwrites all of it that it reads (nothing has to be cleared by the
+ * caller, the previous call's contents never leak into a result), and it is dead once the call's kernels have finished.
+ * Two calls whose kernels can overlap on the GPU (different streams without an event between them, or two host threads
+ * on different streams) RACE on it: serialise them.  Calls on one stream are ordered and safe.
+ * Asynchronous; errors as everywhere (status + message), but the message is per host thread and read with
+ * sc_ivr_fourier_static_last_error() because there is no context to keep it.
+ */
+#define SC_IVR_STATIC_SCRATCH_BYTES (16u << 20)
+size_t sc_ivr_fourier_static_scratch_bytes(long long n, int nsteps, int k);
+sc_ivr_status sc_ivr_fourier_static(const double *z, long long n, int nsteps, double dt, const double *E, int k, double *A_out,
+                                    void *cuda_stream);
+const char *sc_ivr_fourier_static_last_error(void);
+
+/*
  * Parity / debug entry for step a8 through the chirp-z kernels that sc_ivr_run uses on equally spaced grids:
  * P_out[j][i] = | sum_c z[c][j] e^{i E_i c dt} |^2.   z DEVICE [nsteps+1][n][2] (time-major), E HOST [k] equally spaced,
  * P_out DEVICE [n][k], workspace DEVICE sc_ivr_fourier_power_workspace_bytes(ctx, n, k).

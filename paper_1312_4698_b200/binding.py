@@ -23,7 +23,9 @@ EXPORTS = [
     "sc_ivr_propagate", "sc_ivr_eval_pes", "sc_ivr_fourier_workspace_bytes", "sc_ivr_fourier",
     "sc_ivr_fourier_power_workspace_bytes", "sc_ivr_fourier_power", "sc_ivr_multi_workspace_bytes", "sc_ivr_run_multi",
     "sc_ivr_fp64_probe", "sc_ivr_set_timing", "sc_ivr_last_timings", "sc_ivr_last_fallbacks",
+    "sc_ivr_fourier_static", "sc_ivr_fourier_static_scratch_bytes", "sc_ivr_fourier_static_last_error",
 ]
+STATIC_SCRATCH_BYTES = 16 << 20  # SC_IVR_STATIC_SCRATCH_BYTES
 
 
 class sc_ivr_options(C.Structure):
@@ -88,6 +90,12 @@ def lib():
     L.sc_ivr_fourier_power.argtypes = [_vp, _vp, C.c_longlong, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
     L.sc_ivr_fourier.restype = C.c_int
     L.sc_ivr_fourier.argtypes = [_vp, _vp, C.c_longlong, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
+    L.sc_ivr_fourier_static.restype = C.c_int
+    L.sc_ivr_fourier_static.argtypes = [_vp, C.c_longlong, C.c_int, C.c_double, _vp, C.c_int, _vp, _vp]
+    L.sc_ivr_fourier_static_scratch_bytes.restype = C.c_size_t
+    L.sc_ivr_fourier_static_scratch_bytes.argtypes = [C.c_longlong, C.c_int, C.c_int]
+    L.sc_ivr_fourier_static_last_error.restype = C.c_char_p
+    L.sc_ivr_fourier_static_last_error.argtypes = []
     L.sc_ivr_fp64_probe.restype = C.c_int
     L.sc_ivr_fp64_probe.argtypes = [C.c_int, C.c_int, _dp, _dp]
     L.sc_ivr_set_timing.restype = None
@@ -129,6 +137,28 @@ def fp64_probe(mode=0, iters=20000):
     if rc:
         raise ScIvrError(rc, lib().sc_ivr_last_error(None).decode())
     return fl.value, ms.value
+
+
+def fourier_static_scratch_bytes(n, nsteps, k):
+    """sc_ivr_fourier_static_scratch_bytes: what (n, nsteps, k) needs of the STATIC_SCRATCH_BYTES array (0 = out of range)."""
+    return int(lib().sc_ivr_fourier_static_scratch_bytes(int(n), int(nsteps), int(k)))
+
+
+def fourier_static(z, E, dt, A_out):
+    """sc_ivr_fourier_static: A_out[j][i] = sum_c z[c][j] e^{i E_i c dt} for callers that cannot allocate device memory.
+
+    Nothing is allocated, here or in the library: z DEVICE complex128 [nsteps+1, n], E DEVICE float64 [k] and the output
+    A_out DEVICE complex128 [n, k] are all the caller's; the scratch is the library's static array (one per device, shared
+    by every call: do not let two calls overlap on the GPU).  Sizes beyond the array raise ScIvrError(EINVAL)."""
+    import torch
+    assert z.is_cuda and z.dtype == torch.complex128 and z.is_contiguous() and z.dim() == 2
+    assert E.is_cuda and E.dtype == torch.float64 and E.is_contiguous() and E.dim() == 1
+    n, k = z.shape[1], E.shape[0]
+    assert A_out.is_cuda and A_out.dtype == torch.complex128 and A_out.is_contiguous() and tuple(A_out.shape) == (n, k)
+    rc = lib().sc_ivr_fourier_static(_dev(z), n, z.shape[0] - 1, float(dt), _dev(E), k, _dev(A_out), _stream())
+    if rc:
+        raise ScIvrError(rc, lib().sc_ivr_fourier_static_last_error().decode())
+    return A_out
 
 
 class ScIvr:

@@ -14,7 +14,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsc_ivr.so")
-SOURCES = ["api.cu", "propagate_cml.cu", "propagate_tpt.cu", "spectrum.cu", "chirp.cu"]
+SOURCES = ["api.cu", "propagate_cml.cu", "propagate_tpt.cu", "spectrum.cu", "chirp.cu", "fourier_static.cu"]
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "tmem_ldst.cuh"), os.path.join(CSRC, "cml_table.h"),
            os.path.join(HERE, "..", "include", "sc_ivr.h")]
 
