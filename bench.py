@@ -63,10 +63,17 @@ def flop_model(F: int, k: int, det_every_step: bool, morse: bool = False, nsteps
     1386 + 150 + 3888 + 486 + 1980 = 7890, + 3570 with the det M check at every step = 11460.  Fourier stage: the direct
     sum of Eq. 11 is 8k per trajectory-step; on an equally spaced grid the library evaluates it as a chirp-z transform
     (two FFTs of length 8192 per trajectory and block), whose own count 2 * 5 L log2 L * nblocks / (nsteps + 1) is what is
-    credited; nblocks = 0 means the direct sum."""
+    credited; nblocks = 0 means the direct sum.
+
+    Uncoupled Morse oscillators (morse=True) have a DIAGONAL Hessian: each of the 2 F^2 elements of H M_q is one product, not
+    an F-term inner product, and that is all the kernels execute (hessian_times in propagate_cml.cu, the tpt kernel likewise).
+    The monodromy column is therefore 2 (2 F^2 + 6 F^2) = 16 F^2 for them (SURVEY's F = 1 row, 16, generalised), not the
+    dense 2 (2 F^3 + 6 F^2): nothing that is not executed is credited.  The determinant columns stay dense: M_pq, M_qp, 2K and
+    M are eliminated as full matrices whatever the surface (their zero pattern is not exploited), so those flop are executed.
+    The 60 flop per Morse mode count one exp as the survey does."""
     pes = 60 * F if morse else 2 * (F * F * (F + 1) // 2 + 2 * F * F + F * (F - 1) + 6 * F)
     step = 16 * F + 6
-    mono = 2 * (2 * F ** 3 + 6 * F ** 2)
+    mono = 16 * F * F if morse else 2 * (2 * F ** 3 + 6 * F ** 2)
     kmat = 6 * F * F
     cdet = SURVEY_CDET.get(F, 8 * (F - 1) * F * (2 * F - 1) // 6 + 6 * F * (F - 1) // 2 + 16 * F)
     # SURVEY's table also lists ~150 flop-equivalents of transcendentals (exp, sincos, sqrt branch of z_c): this build does

@@ -11,6 +11,11 @@ def test_flop_model_is_the_survey_table():
     assert bench.flop_model(6, 4000, True)["propagate"] == 528 + 102 + 1296 + 216 + 615 + 1012
     assert bench.flop_model(3, 4000, True)["propagate"] == 120 + 54 + 216 + 54 + 95 + 110
     assert bench.flop_model(1, 2000, True, morse=True)["propagate"] == 60 + 22 + 16 + 6 + 10 + 2
+    # uncoupled Morse oscillators, F > 1: diagonal Hessian, so the monodromy column is 16 F^2 (= the F = 1 row's 16 at F = 1), not
+    # the dense 2 (2 F^3 + 6 F^2) that the kernels never execute for them; the determinant columns stay dense
+    assert bench.flop_model(5, 4000, True, morse=True)["propagate"] == 300 + 86 + 400 + 150 + (8 * 4 * 5 * 9 // 6 + 6 * 5 * 4 // 2 + 80) + 570
+    assert bench.flop_model(9, 4000, True, morse=True)["propagate"] == 540 + 150 + 1296 + 486 + 1980 + 3570
+    assert bench.flop_model(9, 4000, True)["propagate"] - bench.flop_model(9, 4000, True, morse=True)["propagate"] == (1386 - 540) + (3888 - 1296)
     # Fourier stage: direct sum 8k, chirp-z two FFTs of length 8192 per trajectory and block
     assert bench.flop_model(9, 4000, True, nblocks=0)["fourier"] == 32000
     one = bench.flop_model(9, 4000, True, nsteps=4000, nblocks=1)["fourier"]
