@@ -143,6 +143,13 @@ struct Cml {
   static constexpr int HMH = ev(C * F);               // parked H dQ: elements per half
   static constexpr int WS = WSG + 2 * HMH * 32;
   static constexpr size_t SMEM = sizeof(double) * (NCOEFP + (size_t)kWarpsC * WS) + 16;
+  // Dynamic shared memory the propagation kernel is LAUNCHED with.  Every CTA takes all 512 columns of the SM's tensor memory,
+  // so a second CTA on the same SM would sit in tcgen05.alloc, holding its slot, until the first one ends, and the launch
+  // shape ("whole rounds of one CTA per SM") would no longer describe what runs.  __launch_bounds__(.., 1) does not cap
+  // residency; shared memory does: two CTAs of more than (228 KB - 2 x 1 KB reserved) / 2 = 113 KB cannot share an SM.  The
+  // small-F rows (F = 4: 113 KB would fit twice) are padded up to that.
+  static constexpr size_t SMEM_ONE_CTA = 115 * 1024;
+  static constexpr size_t SMEM_LAUNCH = SMEM > SMEM_ONE_CTA ? SMEM : SMEM_ONE_CTA;
   __host__ __device__ static constexpr int hm(int e) { return 512 * (e / 2) + 8 * (e % 2); }
 
   // column (l, s) of M: mode a = l + (s % C) L, half h = s / C (0: d/dP0_a, 1: d/dQ0_a), global index h F + a.
@@ -1107,15 +1114,12 @@ __global__ void __launch_bounds__(kThreadsC) k_eval_pes_cml(const double *__rest
 template <int F, int L, int KIND>
 cudaError_t launch_prop_cml(const PropParams &P, cudaStream_t st) {
   using X = Cml<F, L>;
-  static int attr_dev_mask[64] = {0};  // per device: shared-memory opt-in done
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
-  if (dev < 0 || dev >= 64 || !attr_dev_mask[dev]) {
-    e = cudaFuncSetAttribute(k_propagate_cml<F, L, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM);
-    if (e != cudaSuccess) return e;
-    if (dev >= 0 && dev < 64) attr_dev_mask[dev] = 1;
-  }
+  // per device and cheap: set on every launch, no process-wide flag (as chirp.cu and spectrum.cu do)
+  e = cudaFuncSetAttribute(k_propagate_cml<F, L, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)X::SMEM_LAUNCH);
+  if (e != cudaSuccess) return e;
   int sm = 0;
   e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
   if (e != cudaSuccess) return e;
@@ -1128,7 +1132,7 @@ cudaError_t launch_prop_cml(const PropParams &P, cudaStream_t st) {
   Q.cta_full = (int)full;
   Q.cta_warps = tail ? (int)(left / tail) : 0;
   Q.cta_warps_rem = tail ? (int)(left % tail) : 0;
-  k_propagate_cml<F, L, KIND><<<(unsigned)(full + tail), kThreadsC, X::SMEM, st>>>(Q);
+  k_propagate_cml<F, L, KIND><<<(unsigned)(full + tail), kThreadsC, X::SMEM_LAUNCH, st>>>(Q);
   return cudaGetLastError();
 }
 
