@@ -541,3 +541,31 @@ def test_combo_reference_state_brute_force(oracle):
     Ib, ngb = brute.spectrum_combo(pes, w.gamma, w.dt, w.nsteps, w.p0q0, chis, eps, w.E)
     assert ng == ngb == 5 and rc == 0
     assert np.max(np.abs(I - Ib)) < 1e-11 * Ib.max()
+
+
+def test_r22_flag_is_decided_by_roundoff(oracle):
+    """Reading R22: tests/golden/r22_flag.txt holds, for trajectory 105793 of config 5, the determinant of
+    the oracle's own monodromy matrix evaluated in 60-digit arithmetic (make_r22_flag.py).  The exact map has det M = 1
+    (PAPER.md:64), so what the file lists is accumulated round-off: negligible while eps max|M|^2 << det_tol, of the size of
+    det_tol = 1e-6 once max|M| >= 1e6.  That is the regime in which the GPU parity test lets at most two flags
+    differ.  The file is tied to the oracle as it stands: max|M| and the flag are recomputed here."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "r22_flag.txt")
+    rows = np.array([[float(x) for x in ln.split()] for ln in open(path) if not ln.startswith("#")])
+    assert rows.shape[1] == 6 and rows[-1, 0] == 8000
+    nsteps, good, mmax, dev_exact, dev_f64, bound = rows.T
+    tol = 1e-6
+    early = bound < 1e-1 * tol                       # the flag is a property of the trajectory: far inside the tolerance, accepted
+    assert early.sum() >= 2 and np.all(dev_exact[early] < 1e-3 * tol) and np.all(good[early] == 1)
+    late = mmax >= 1e6                               # the flag is round-off: deviation within a factor 30 of the tolerance either way
+    assert late.sum() >= 3 and np.all(bound[late] > 100 * tol)
+    assert np.all((dev_exact[late] > tol / 30) & (dev_exact[late] < tol * 30))
+    assert dev_exact[late].min() < tol < dev_exact[late].max()   # both sides of it along one trajectory
+    assert np.all(good[dev_exact > tol] == 0)        # the oracle rejects where the determinant of ITS M is outside (rightly)
+    assert np.all(np.abs(dev_f64 - dev_exact) <= 1e3 * bound)    # and a double-precision determinant of that M is no better than eps max|M|^2
+    # the same trajectory through today's oracle
+    w = inputs.make_config(5, ntraj=1 << 17, nsteps=8000)
+    pq = np.ascontiguousarray(w.p0q0[:, 105793:105794])
+    for i in (1, len(rows) - 1):
+        po = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, int(nsteps[i]), pq, want_M=True)
+        assert abs(np.abs(po["M"]).max() - mmax[i]) <= 1e-8 * mmax[i]
+        assert int(po["good"][0]) == int(good[i])
