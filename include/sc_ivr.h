@@ -176,6 +176,19 @@ sc_ivr_status sc_ivr_propagate(sc_ivr_ctx *ctx, const double *p0q0, long long nt
                                void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /*
+ * Parity / debug entry for the z assembly alone (the branch rule of a5, a6 and the input of a8): from the per-step records that
+ * the propagation kernel writes to the z_{j,c} of Eq. 11, by the kernel sc_ivr_propagate and the direct-sum
+ * path of sc_ivr_run use.
+ *   raw       DEVICE [nsteps_run+1][n][4]: (ln|<chi|pq>|, S + arg<chi|pq>, Re D, Im D), D = det 2K times ANY positive factor
+ *             (only its phase is used; components from subnormal up to the largest finite double are handled)
+ *   z_out     DEVICE [nsteps_run+1][n][2]:  exp(raw0) e^{i raw1} u_c,  u_c = the square root of D_c / |D_c| on the branch that is
+ *             continuous in c, u_0 the principal one
+ *   theta_out DEVICE [n] or NULL: the unwrapped arg D at the last step
+ */
+sc_ivr_status sc_ivr_assemble_z(sc_ivr_ctx *ctx, const double *raw, long long n, int nsteps_run, double *z_out,
+                                double *theta_out, void *cuda_stream);
+
+/*
  * Parity / debug entry for step a1: the potential, its gradient and Hessian, evaluated by the same
  * device code the propagation kernel inlines.   q DEVICE [F][n] -> V_out [n], g_out [F][n], H_out [F][F][n].
  */

@@ -23,7 +23,7 @@ EXPORTS = [
     "sc_ivr_propagate", "sc_ivr_eval_pes", "sc_ivr_fourier_workspace_bytes", "sc_ivr_fourier",
     "sc_ivr_fourier_power_workspace_bytes", "sc_ivr_fourier_power", "sc_ivr_multi_workspace_bytes", "sc_ivr_run_multi",
     "sc_ivr_fp64_probe", "sc_ivr_set_timing", "sc_ivr_last_timings", "sc_ivr_last_fallbacks",
-    "sc_ivr_fourier_static", "sc_ivr_fourier_static_scratch_bytes", "sc_ivr_fourier_static_last_error",
+    "sc_ivr_fourier_static", "sc_ivr_fourier_static_scratch_bytes", "sc_ivr_fourier_static_last_error", "sc_ivr_assemble_z",
 ]
 STATIC_SCRATCH_BYTES = 16 << 20  # SC_IVR_STATIC_SCRATCH_BYTES
 
@@ -90,6 +90,8 @@ def lib():
     L.sc_ivr_fourier_power.argtypes = [_vp, _vp, C.c_longlong, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
     L.sc_ivr_fourier.restype = C.c_int
     L.sc_ivr_fourier.argtypes = [_vp, _vp, C.c_longlong, _dp, C.c_int, _vp, _vp, C.c_size_t, _vp]
+    L.sc_ivr_assemble_z.restype = C.c_int
+    L.sc_ivr_assemble_z.argtypes = [_vp, _vp, C.c_longlong, C.c_int, _vp, _vp, _vp]
     L.sc_ivr_fourier_static.restype = C.c_int
     L.sc_ivr_fourier_static.argtypes = [_vp, C.c_longlong, C.c_int, C.c_double, _vp, C.c_int, _vp, _vp]
     L.sc_ivr_fourier_static_scratch_bytes.restype = C.c_size_t
@@ -289,6 +291,16 @@ class ScIvr:
         H = torch.empty((F, F, n), dtype=torch.float64, device=dev)
         self._check(lib().sc_ivr_eval_pes(self._h, _dev(q), n, _dev(V), _dev(g), _dev(H), _stream()))
         return V, g, H
+
+    def assemble_z(self, raw, want_theta=True):
+        """sc_ivr_assemble_z: raw DEVICE float64 [nsteps_run+1, n, 4] -> (z DEVICE complex [nsteps_run+1, n], theta [n] or None)."""
+        import torch
+        assert raw.is_cuda and raw.dtype == torch.float64 and raw.is_contiguous() and raw.dim() == 3 and raw.shape[2] == 4
+        rows, n = raw.shape[0], raw.shape[1]
+        z = torch.empty((rows, n, 2), dtype=torch.float64, device=raw.device)
+        th = torch.empty(n, dtype=torch.float64, device=raw.device) if want_theta else None
+        self._check(lib().sc_ivr_assemble_z(self._h, _dev(raw), n, rows - 1, _dev(z), _dev(th), _stream()))
+        return torch.view_as_complex(z), th
 
     def _lib_multi_bytes(self, ntraj, k, ncs, max_batch=0):
         return int(lib().sc_ivr_multi_workspace_bytes(self._h, int(ntraj), int(k), int(ncs), int(max_batch)))

@@ -575,6 +575,17 @@ sc_ivr_status sc_ivr_propagate(sc_ivr_ctx *ctx, const double *p0q0, long long nt
   return SC_IVR_OK;
 }
 
+sc_ivr_status sc_ivr_assemble_z(sc_ivr_ctx *ctx, const double *raw, long long n, int nsteps_run, double *z_out, double *theta_out,
+                                void *cuda_stream) {
+  if (!ctx) return SC_IVR_EINVAL;
+  if (sc_ivr_status ds = check_device(ctx)) return ds;
+  if (!raw || !z_out) return fail(ctx, SC_IVR_EINVAL, "NULL argument");
+  if (n < 1 || nsteps_run < 0) return fail(ctx, SC_IVR_EINVAL, "n must be >= 1 and nsteps_run >= 0");
+  CU(sci_launch_zassemble((const double4 *)raw, n, n, nsteps_run, (double2 *)z_out, n, n, nsteps_run + 1, theta_out,
+                          (cudaStream_t)cuda_stream));
+  return SC_IVR_OK;
+}
+
 sc_ivr_status sc_ivr_eval_pes(sc_ivr_ctx *ctx, const double *q, long long n, double *V_out, double *g_out, double *H_out,
                               void *cuda_stream) {
   if (!ctx) return SC_IVR_EINVAL;

@@ -136,14 +136,21 @@ cudaError_t sci_launch_chirp_fft(int mode, const double2 *x, long long xstride, 
 #ifdef __CUDACC__
 // 1 / |D| for D = (re, im) without overflow or underflow of the squares: the determinant record carries an arbitrary positive
 // factor (the static elimination hands over det 2K times |prod 1/pivot|^2), so it is brought to unit scale by a power of two
-// taken from the larger component's exponent before it is squared (the oracle uses cabs)
+// taken from the larger component's exponent before it is squared (the oracle uses cabs).  The power 2^(1023 - ex) is a normal
+// double for every ex <= 0x7fd, subnormal inputs (ex = 0) included: they come out in [2^-51, 2), whose squares are far from
+// underflow.  For ex = 0x7fe (|D| >= 2^1023) it would be 2^-1023, which is not, so such a record is quartered first.  ex = 0x7ff
+// (inf, NaN) yields NaN, as it must: that trajectory is rejected by the finite check of a7.  D = 0 exactly yields NaN too (det K
+// = 0 has no phase; the oracle's division by cabs = 0 does the same).
 __device__ __forceinline__ double unit_scale(double &re, double &im) {
-  const int ex = (int)((max((unsigned)__double2hiint(re) & 0x7fffffffu, (unsigned)__double2hiint(im) & 0x7fffffffu) >> 20) & 0x7ffu);
-  if (ex > 0 && ex < 0x7fe) {
-    const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex)
-    re *= sc;
-    im *= sc;
+  int ex = (int)((max((unsigned)__double2hiint(re) & 0x7fffffffu, (unsigned)__double2hiint(im) & 0x7fffffffu) >> 20) & 0x7ffu);
+  if (ex >= 0x7fe) {
+    re *= 0.25;
+    im *= 0.25;
+    ex -= 2;
   }
+  const double sc = __hiloint2double((0x7fe - ex) << 20, 0);  // 2^(1023 - ex)
+  re *= sc;
+  im *= sc;
   return 1.0 / sqrt(fma(re, re, im * im));
 }
 #endif

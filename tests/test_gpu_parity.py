@@ -340,6 +340,44 @@ def test_run_parity_config1_full(torch_cuda, B, oracle):
     _assert_spectrum(oracle, I, Io)
 
 
+def test_run_parity_config2_full(torch_cuda, B, oracle):
+    """Config 2 at its full size with every weight 1: 16384 trajectories x 4000 steps, 4000 energies, the launch bench.py
+    --config 2 times, against the oracle's whole spectrum (about a minute of the box's host cores).  Covers what the sampled
+    full-size test cannot: the accumulation over all trajectories of a chirp-z CTA and the final sum over the CTAs' partial rows
+    (north star "on all 5 configs").  Configs 3 and 4 in full: bench.py --verify-full, profiles/r03_full_parity.md."""
+    w = inputs.make_config(2)
+    assert (w.ntraj, w.nsteps, w.k) == (16384, 4000, 4000)
+    I, ng, rc, Io, ngo, rco = _run_both(torch_cuda, B, oracle, w)
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I, Io)
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_run_parity_config3_config4_full(torch_cuda, B, oracle, cfg):
+    """Configs 3 and 4 at their full sizes with every weight 1 against the oracle's whole spectrum: about 4 and 11 minutes of the
+    box's host cores, so the test only runs when SC_IVR_FULL_PARITY=1 is set (profiles/r03_full_parity.md holds the record of
+    the round-3 run; command there).  Prints one line per config and appends it to gpurun_out/full_parity.txt."""
+    import os
+    import time
+    if os.environ.get("SC_IVR_FULL_PARITY") != "1":
+        pytest.skip("set SC_IVR_FULL_PARITY=1 (the oracle needs 4 + 11 minutes)")
+    w = inputs.make_config(cfg)
+    t0 = time.perf_counter()
+    I, ng, rc, Io, ngo, rco = _run_both(torch_cuda, B, oracle, w)
+    err = float(np.max(np.abs(I - Io)) / Io.max())
+    pk, pko = oracle.find_peaks(I), oracle.find_peaks(Io)
+    line = (f"{w.name}: F={w.F} ntraj={w.ntraj} nsteps={w.nsteps} k={w.k}  n_good gpu/oracle={ng}/{ngo}  rc={rc}/{rco}  "
+            f"max|I-I_oracle|/max(I_oracle)={err:.3e}  peak bins gpu/oracle={len(pk)}/{len(pko)} identical={np.array_equal(pk, pko)}  "
+            f"wall={time.perf_counter() - t0:.0f}s")
+    print(line)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    if os.path.isdir(os.path.join(root, "gpurun_out")):
+        with open(os.path.join(root, "gpurun_out", "full_parity.txt"), "a") as f:
+            f.write(line + "\n")
+    assert (ng, rc) == (ngo, rco)
+    _assert_spectrum(oracle, I, Io)
+
+
 @pytest.mark.parametrize("cfg,ntraj", [(2, 300), (3, 200), (4, 150)])
 def test_run_parity_configs_full_time_and_energy_grid(torch_cuda, B, oracle, cfg, ntraj):
     """Configs 2-4 with their full time and energy grids (4000 steps, 4000 energies) on a trajectory
@@ -424,18 +462,22 @@ def test_error_paths(torch_cuda, B):
     assert e.value.status == B.EINVAL and "workspace" in str(e.value)
 
 
-def _layout_picks(w, n_random, seed):
+def _layout_picks(w, n_random, seed, wave, sm_count):
     """Sampled trajectories of a full-size run: random ones plus the places where the launch layout has its seams (first
     and last trajectory of a warp group and of a CTA, both sides of a batch boundary, the start of the last, partial
-    round of CTAs, the very last trajectory)."""
+    round of CTAs, the very last trajectory).  The layout comes from the library, not from a table typed in here: `wave` =
+    sc_ivr_min_batch = the trajectories one round of CTAs holds on `sm_count` SMs, so wave / sm_count is what one SM holds at a
+    time (one CTA of the lanes-per-trajectory kernels; a few 128-thread CTAs of the thread-per-trajectory kernels), and its
+    halves down to an eighth are the CTA's warps (8 per CTA) and the CTAs of an SM."""
     n = w.ntraj
     rng = np.random.default_rng(seed)
     pick = set(rng.choice(n, n_random, replace=False).tolist())
-    lanes = {9: 3, 6: 2, 3: 1}.get(w.F, 1)
-    G = 32 // lanes if w.F > 3 else 128          # trajectories per warp (thread-per-trajectory kernels: per CTA)
-    cta = 8 * G if w.F > 3 else 128
-    wave = 148 * cta
-    seams = [0, G - 1, G, cta - 1, cta, wave - 1, wave, (n // wave) * wave - 1, (n // wave) * wave, 131071, 131072, n - G, n - 2, n - 1]
+    assert wave > 0 and wave % sm_count == 0
+    per_sm = wave // sm_count
+    units = sorted({32, 128, per_sm} | {per_sm // d for d in (2, 4, 8) if per_sm % d == 0})
+    seams = [0, wave - 1, wave, (n // wave) * wave - 1, (n // wave) * wave, 131071, 131072, n - 2, n - 1]
+    for u in units:
+        seams += [u - 1, u, n - u]
     pick |= {j for j in seams if 0 <= j < n}
     return np.array(sorted(pick))
 
@@ -453,21 +495,26 @@ def test_full_size_sampled_trajectories(torch_cuda, B, oracle, cfg, ntraj, nstep
     w = inputs.make_config(cfg, ntraj=ntraj, nsteps=nsteps)
     ctx = B.ScIvr.from_workload(w)
     d_pq = _dev(torch, w.p0q0)
-    pick = _layout_picks(w, 16, 99 + cfg)
+    pick = _layout_picks(w, 16, 99 + cfg, ctx.min_batch(), torch.cuda.get_device_properties(0).multi_processor_count)
     if cfg == 5 and w.nsteps > 4000:
         # long runs reject trajectories (|det M - 1| > 1e-6 after 8000 steps of a chaotic one): every rejected trajectory of
         # the device run joins the sample and the oracle must reject the same ones.  Where M has grown to ~1e6 the flag is
         # defined by round-off on either side (the two states differ by eps x stretching, det M - 1 is a difference of
         # 1e12-sized terms): such a trajectory may differ and leaves the sample; at most two do
-        bad = np.flatnonzero(ctx.propagate(d_pq, w.nsteps, want_M=False, want_theta=False)["good"].cpu().numpy() == 0)
+        good_dev = ctx.propagate(d_pq, w.nsteps, want_M=False, want_theta=False)["good"].cpu().numpy()
+        bad = np.flatnonzero(good_dev == 0)
         assert 0 < len(bad) <= 64
         pick = np.array(sorted(set(pick.tolist()) | set(bad.tolist())))
-        po = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, np.ascontiguousarray(w.p0q0[:, pick]), want_M=True)
-        bad_o = pick[po["good"] == 0]
-        disputed = sorted(set(bad.tolist()) ^ set(bad_o.tolist()))
+        # flags: the oracle decides them for the sample, for every trajectory the device rejected AND for 2048 random ones,
+        # so that a trajectory the device accepts and the oracle rejects does not go unnoticed outside the sample
+        extra = np.random.default_rng(7).choice(w.ntraj, 2048, replace=False)
+        chk = np.array(sorted(set(pick.tolist()) | set(extra.tolist())))
+        po = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, np.ascontiguousarray(w.p0q0[:, chk]), want_M=True)
+        bad_o = chk[po["good"] == 0]
+        disputed = sorted(set(chk[good_dev[chk] == 0].tolist()) ^ set(bad_o.tolist()))
         assert len(disputed) <= 2
         for j in disputed:
-            assert np.abs(po["M"][..., int(np.flatnonzero(pick == j)[0])]).max() >= 1e6, f"flag of trajectory {j} differs"
+            assert np.abs(po["M"][..., int(np.flatnonzero(chk == j)[0])]).max() >= 1e6, f"flag of trajectory {j} differs"
         pick = np.array([j for j in pick.tolist() if j not in disputed])
         n_bad = len(bad)
         n_bad_pick = len([j for j in bad.tolist() if j not in disputed])
@@ -488,10 +535,10 @@ def test_full_size_sampled_trajectories(torch_cuda, B, oracle, cfg, ntraj, nstep
 
 
 @pytest.mark.parametrize("world", [2, 3])
-def test_shards_of_a_real_run_recombine(torch_cuda, B, world):
+def test_shards_of_a_real_run_recombine(torch_cuda, B, oracle, world):
     """Rows e / f5 on one GPU: sc_ivr_run on the blocks shard_bounds gives each rank, one
     block holding a poisoned trajectory so that its n_good differs, combined with the arithmetic of combine_spectra
-    (Eq. 11's 1 / n_good is per job), against the unsharded run."""
+    (Eq. 11's 1 / n_good is per job), against the unsharded run and against the oracle."""
     from paper_1312_4698_b200.sharding import combine_shards, combine_spectra, shard_bounds
     torch = torch_cuda
     w = inputs.make_config(4, ntraj=331, nsteps=300, k=200)
@@ -511,6 +558,48 @@ def test_shards_of_a_real_run_recombine(torch_cuda, B, world):
     I, ng = combine_shards(parts, ngs)
     assert ng == ng_all
     assert float((I - I_all).abs().max()) <= 1e-13 * float(I_all.max())
+    # and against the oracle on the same inputs (it rejects the poisoned trajectory too): the recombined shards ARE Eq. 11
+    Io, ngo, rco = oracle.run(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, pq, w.chi, w.E)
+    assert (ngo, rco) == (330, 0)
+    _assert_spectrum(oracle, I.cpu().numpy(), Io)
     # the collective entry point with no process group is the one-shard case of the same sum
     I1, ng1 = combine_spectra(I_all, ng_all)
     assert ng1 == ng_all and float((I1 - I_all).abs().max()) <= 4e-16 * float(I_all.max())  # x n / n
+
+
+def test_z_assembly_with_extreme_determinant_records(torch_cuda, B):
+    """a5 branch rule + a6 through sc_ivr_assemble_z when det 2K arrives at any scale: the record carries the determinant times an
+    arbitrary positive factor and only its phase may matter (Eq. 11; branch continuity PAPER.md:86).  Components from
+    subnormal (1e-320) through 1 to beyond 2^1023 (1.7e308), where squaring the record would underflow or overflow and where the
+    power of two that brings it to unit scale is itself not a normal double.  Reference: the same definition in numpy with the
+    components rescaled exactly (ldexp) before the modulus is taken."""
+    torch = torch_cuda
+    rng = np.random.default_rng(21)
+    rows, n = 60, 37
+    mags = np.array([1e-320, 2.3e-310, 4e-308, 1e-300, 1e-150, 1.0, 1e150, 1e300, 9.1e307, 1.7e308])
+    mag = mags[(np.arange(rows)[:, None] * 3 + np.arange(n)[None, :]) % mags.size]
+    phi = rng.uniform(-np.pi, np.pi, n)[None, :] + 0.3 * np.arange(rows)[:, None] + 0.05 * rng.standard_normal((rows, n))
+    raw = np.empty((rows, n, 4))
+    raw[..., 0] = rng.uniform(-3.0, 0.0, (rows, n))
+    raw[..., 1] = rng.uniform(-50.0, 50.0, (rows, n))
+    raw[..., 2] = mag * np.cos(phi)
+    raw[..., 3] = mag * np.sin(phi)
+    assert np.isfinite(raw).all() and np.abs(raw[..., 2:]).max() > 2.0 ** 1023 and 0 < np.abs(raw[..., 2:]).min() < 2.3e-308
+    w = inputs.make_config(1, ntraj=2, nsteps=rows - 1, k=8)
+    z, th = B.ScIvr.from_workload(w).assemble_z(_dev(torch, raw))
+    z, th = z.cpu().numpy(), th.cpu().numpy()
+    # definition
+    _, e = np.frexp(np.maximum(np.abs(raw[..., 2]), np.abs(raw[..., 3])))
+    re, im = np.ldexp(raw[..., 2], -e), np.ldexp(raw[..., 3], -e)
+    ph = (re + 1j * im) / np.hypot(re, im)
+    u = np.sqrt(ph)                                   # principal root
+    for c in range(1, rows):
+        flip = (u[c] * np.conj(u[c - 1])).real < 0.0
+        u[c] = np.where(flip, -u[c], u[c])
+    zo = np.exp(raw[..., 0]) * np.exp(1j * raw[..., 1]) * u
+    assert np.isfinite(z).all()
+    assert np.max(np.abs(z - zo)) < 1e-12
+    arg = np.angle(ph)
+    d = np.diff(np.concatenate([np.zeros((1, n)), arg]), axis=0)
+    d = (d + np.pi) % (2 * np.pi) - np.pi
+    assert np.max(np.abs(th - d.sum(axis=0))) < 1e-10
