@@ -314,6 +314,45 @@ def test_run_uncoupled_morse_oscillators(torch_cuda, B, oracle, F):
     _assert_spectrum(oracle, I, Io)
 
 
+# (config, trajectory of the 2^17-row draw, first step at which the fixed-order elimination of det M misses the tolerance):
+# found by a search over all 2^17 trajectories x 8000 steps with the multiplier guard off; at these steps max|M| is 5e2 .. 1e4
+# and the oracle's |det M - 1| is 1e-12 .. 1e-14, so the flag is a property of the trajectory (not the round-off regime of R22)
+# The same search over the 2^17-row draws of configs 2 and 3 (F = 3, 6) found no such step within 8000: the copy of the rule in
+# the thread-per-trajectory kernels is reached only through the forced / mixed fallback tests above.
+SUSPECT_CASES = [(5, 116626, 3492), (5, 34265, 4645), (5, 24747, 4718)]
+
+
+@pytest.mark.parametrize("cfg,j,first", SUSPECT_CASES)
+def test_static_order_rejection_is_confirmed_by_the_pivoted_elimination(torch_cuda, B, oracle, cfg, j, first):
+    """a7: a trajectory is only ever rejected by the PIVOTED elimination.  With lu_growth_max = 1e99 the
+    multiplier guard never fires, so the only way into the pivoted routines is the rule "the fixed order is about to reject":
+    at step `first` of trajectory j the fixed-order det M is off by more than 1e-6 (a pivot passes through zero) although M is
+    benign.  Expected, deterministically: exactly one repeated trajectory-step, the trajectory accepted as the oracle accepts
+    it, the spectrum equal to the oracle's; one step earlier no repeat at all; the default guard gives the same flags."""
+    torch = torch_cuda
+    w = inputs.make_config(cfg, ntraj=1 << 17, nsteps=first + 8, k=64)
+    pq = np.ascontiguousarray(w.p0q0[:, [j - 1, j, j + 1]])         # the neighbours are ordinary trajectories
+    po = oracle.propagate(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, first, pq[:, 1:2], want_M=True)
+    Mb = po["M"][..., 0]
+    M = np.block([[Mb[0], Mb[1]], [Mb[2], Mb[3]]])
+    assert po["good"][0] == 1 and np.abs(M).max() < 1e5 and abs(np.linalg.det(M) - 1.0) < 1e-9   # the flag is well determined
+    Io, ngo, rco = oracle.run(w.F, w.pes_kind, w.pes_coeffs, w.gamma, w.dt, w.nsteps, pq, w.chi, w.E)
+    assert (ngo, rco) == (3, 0)
+    ctx = B.ScIvr.from_workload(w, lu_growth_max=1e99)
+    I, ng, rc = ctx.run(_dev(torch, pq), w.chi, w.E)
+    assert (ng, rc) == (3, 0) and ctx.last_fallbacks() == 1
+    _assert_spectrum(oracle, I.cpu().numpy(), Io)
+    assert bool(ctx.propagate(_dev(torch, pq), w.nsteps, want_M=False, want_theta=False)["good"].cpu().numpy().all())
+    w0 = inputs.make_config(cfg, ntraj=1 << 17, nsteps=first - 1, k=64)
+    ctx0 = B.ScIvr.from_workload(w0, lu_growth_max=1e99)
+    _, ng0, rc0 = ctx0.run(_dev(torch, pq), w0.chi, w0.E)
+    assert (ng0, rc0) == (3, 0) and ctx0.last_fallbacks() == 0
+    ctxd = B.ScIvr.from_workload(w)                                  # default guard (1e4): same decision, by whichever rule
+    Id, ngd, rcd = ctxd.run(_dev(torch, pq), w.chi, w.E)
+    assert (ngd, rcd) == (3, 0) and ctxd.last_fallbacks() >= 1
+    _assert_spectrum(oracle, Id.cpu().numpy(), Io)
+
+
 def _run_both(torch, B, oracle, w, **kw):
     ctx = B.ScIvr.from_workload(w, **kw)
     I, ng, rc = ctx.run(_dev(torch, w.p0q0), w.chi, w.E)
