@@ -324,6 +324,20 @@ def main():
             probe = {"dfma_tflops": B.fp64_probe(0, 20000)[0] / 1e12, "dmma_tflops": B.fp64_probe(1, 20000)[0] / 1e12}
         except Exception as ex:  # measurement helper only
             probe = {"error": str(ex)}
+        try:
+            # issue-budget probes (kernel A "what bounds it"): DFMA rate alone and with a shuffle / LDS after every 4
+            # DFMAs or an integer pair after every DFMA, at 16, 2 and 1 warps per scheduler (kernel A runs at 2); only DFMAs count.
+            # cycles = SM clock x 4 schedulers x SMs / DFMA warp-instructions per second
+            sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+            mhz = clocks.get("sm_mhz") or 1965.0
+            issue = {}
+            for name, mode in (("dfma_16wps", 0), ("dfma_2wps", 20), ("dfma_shfl_2wps", 22), ("dfma_lds_2wps", 23), ("dfma_int_2wps", 24),
+                               ("dfma_1wps", 10), ("dfma_shfl_1wps", 12), ("dfma_lds_1wps", 13), ("dfma_int_1wps", 14)):
+                tf = B.fp64_probe(mode, 20000)[0] / 1e12
+                issue[name] = {"dfma_tflops": tf, "cycles_per_dfma_per_scheduler": mhz * 1e6 * 4 * sms * 64 / (tf * 1e12)}
+            probe["issue"] = issue
+        except Exception as ex:  # measurement helper only
+            probe["issue"] = {"error": str(ex)}
         cpu = None
         if not args.no_cpu_baseline:
             cpu, _ = cpu_oracle_sample(w, args.ref_sample, args.det_stride, args.integrator)

@@ -247,6 +247,10 @@ sc_ivr_status sc_ivr_fourier_power(sc_ivr_ctx *ctx, const double *z, long long n
  * Measurement helpers (no method arithmetic).
  * sc_ivr_fp64_probe: runs a register-only DFMA loop (mode 0) or an mma.sync m8n8k4 f64 loop (mode 1)
  * on every SM and returns the achieved FLOP/s (2 flop per FMA) in *flops_out.  Synchronous.
+ * Issue-budget probes, mode = kind + 10 * wps: kind 2 = the DFMA loop with a 64-bit warp shuffle after every 4 DFMAs, 3 = with
+ * an LDS.64 after every 4, 4 = with an integer LOP3 / IADD3 pair after every DFMA (only the DFMAs count as flop: a rate equal to
+ * kind 0's means the extra instruction issued in the FP64 pipe's shadow); wps 0 = 16 warps per scheduler, 1 or 2 = exactly that
+ * many (one CTA of 128 or 256 threads per SM), which is the occupancy kernel A runs at.  Other modes: SC_IVR_EINVAL.
  * sc_ivr_last_timings: device times in ms (CUDA events on the run stream) of the stages of the most
  * recent sc_ivr_run on ctx, summed over batches: [0] propagate kernel, [1] z assembly, [2] twiddle / chirp tables,
  * [3] Fourier kernel (direct sum or chirp-z), [4] reduction kernels; [5] number of kernel launches.  Synchronises the stream's

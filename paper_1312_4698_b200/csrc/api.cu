@@ -376,7 +376,8 @@ sc_ivr_status sc_ivr_last_timings(sc_ivr_ctx *ctx, double out[6]) {
 
 sc_ivr_status sc_ivr_fp64_probe(int mode, int iters, double *flops_out, double *ms_out) {
   sc_ivr_ctx *ctx = nullptr;
-  if (!flops_out || !ms_out || iters < 1 || (mode != 0 && mode != 1)) return fail(ctx, SC_IVR_EINVAL, "bad probe arguments");
+  if (!flops_out || !ms_out || iters < 1 || mode < 0 || mode % 10 > 4 || mode / 10 > 2)
+    return fail(ctx, SC_IVR_EINVAL, "bad probe arguments (mode = kind 0..4 + 10 x warps per scheduler 0..2)");
   CU(sci_fp64_probe(mode, iters, flops_out, ms_out));
   return SC_IVR_OK;
 }

@@ -265,6 +265,48 @@ __global__ void __launch_bounds__(256) k_probe_dmma(int iters, double *out) {
   if (s == 12345.678) out[0] = s;
 }
 
+// Issue-budget probes (kernel A "what bounds it"): the DFMA loop of k_probe_dfma with ONE other instruction after every
+// NF DFMAs, so that the time per DFMA says whether that instruction issues in the shadow of the FP64 pipe or takes a slot of its own.
+//   MIX 2: a 64-bit warp shuffle (two SHFL.IDX) every 4 DFMAs     MIX 3: an LDS.64 every 4 DFMAs (its value is the next addend)
+//   MIX 4: one integer LOP3 / IADD3 pair after EVERY DFMA
+// Only the DFMAs are counted as flop.
+template <int MIX>
+__global__ void __launch_bounds__(256) k_probe_mix(int iters, double *out) {
+  __shared__ double tab[512];
+  tab[threadIdx.x] = 1e-9 * (threadIdx.x + 1);
+  tab[256 + threadIdx.x] = 2e-9 * (threadIdx.x + 1);
+  __syncthreads();
+  // nothing but the DFMA chains themselves is a dependent chain: a loaded value is first used a whole iteration (16 DFMAs)
+  // later, the 16 integer counters are independent of one another, a shuffled accumulator is next touched 13 DFMAs later
+  double a[16], yv[4];
+  unsigned k[16];
+  const double x = 1.0 + 1e-9 * threadIdx.x;
+#pragma unroll
+  for (int i = 0; i < 16; i++) {
+    a[i] = (double)i;
+    k[i] = threadIdx.x + i;
+  }
+#pragma unroll
+  for (int i = 0; i < 4; i++) yv[i] = 1e-9;
+  for (int it = 0; it < iters; it++) {
+    double yn[4] = {yv[0], yv[1], yv[2], yv[3]};
+    const double *tp = tab + ((threadIdx.x + it) & 255);
+#pragma unroll
+    for (int i = 0; i < 16; i++) {
+      a[i] = fma(a[i], x, yv[i >> 2]);
+      if (MIX == 2 && (i & 3) == 3) a[i - 3] = __shfl_xor_sync(0xffffffffu, a[i - 3], 1);
+      if (MIX == 3 && (i & 3) == 3) yn[i >> 2] = tp[i];
+      if (MIX == 4) k[i] = (k[i] ^ (unsigned)it) + (unsigned)i;
+    }
+#pragma unroll
+    for (int i = 0; i < 4; i++) yv[i] = yn[i];
+  }
+  double s = yv[0] + yv[1] + yv[2] + yv[3];
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += a[i] + (double)(k[i] & 1u);
+  if (s == 12345.678) out[0] = s;
+}
+
 }  // namespace
 
 cudaError_t sci_launch_zassemble(const double4 *raw, long long raw_stride, long long nb, int nsteps, double2 *z,
@@ -320,11 +362,23 @@ cudaError_t sci_fp64_probe(int mode, int iters, double *flops, double *ms_out) {
   cudaEvent_t a, b;
   cudaEventCreate(&a);
   cudaEventCreate(&b);
-  const int blocks = sms * 8, threads = 256;
+  // mode = kind + 10 * wps.  kind: 0 DFMA, 1 DMMA, 2 DFMA + SHFL, 3 DFMA + LDS, 4 DFMA + integer.  wps: 0 = 16 warps per scheduler
+  // (8 CTAs of 256 threads per SM), 1 or 2 = that many warps per scheduler (one CTA of 128 or 256 threads per SM)
+  const int kind = mode % 10, wps = mode / 10;
+  if (kind > 4 || wps > 2 || mode < 0) {
+    cudaFree(d);
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    return cudaErrorInvalidValue;
+  }
+  const int blocks = wps == 0 ? sms * 8 : sms, threads = wps == 1 ? 128 : 256;
   for (int rep = 0; rep < 2; rep++) {  // first pass is the warm-up
     cudaEventRecord(a);
-    if (mode == 0) k_probe_dfma<<<blocks, threads>>>(iters, d);
-    else k_probe_dmma<<<blocks, threads>>>(iters, d);
+    if (kind == 0) k_probe_dfma<<<blocks, threads>>>(iters, d);
+    else if (kind == 1) k_probe_dmma<<<blocks, threads>>>(iters, d);
+    else if (kind == 2) k_probe_mix<2><<<blocks, threads>>>(iters, d);
+    else if (kind == 3) k_probe_mix<3><<<blocks, threads>>>(iters, d);
+    else k_probe_mix<4><<<blocks, threads>>>(iters, d);
     cudaEventRecord(b);
     e = cudaEventSynchronize(b);
     if (e != cudaSuccess) break;
@@ -335,7 +389,7 @@ cudaError_t sci_fp64_probe(int mode, int iters, double *flops, double *ms_out) {
   cudaEventDestroy(b);
   cudaFree(d);
   if (e != cudaSuccess) return e;
-  const double fl = mode == 0 ? 2.0 * 16.0 * (double)iters * blocks * threads
+  const double fl = kind != 1 ? 2.0 * 16.0 * (double)iters * blocks * threads
                               : 2.0 * 8.0 * 8 * 8 * 4 * (double)iters * blocks * (threads / 32);
   *flops = fl / (ms * 1e-3);
   *ms_out = ms;
